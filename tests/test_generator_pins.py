@@ -1,0 +1,163 @@
+"""Pins for the seeded input generator.
+
+The generator serves both the oracle and the CUDA path, so it is pinned
+against the paper's printed numbers (Table 2 n_ik), the paper's structural
+identities (Eq. 22, 24a, 25) and closed forms (two-level G, G(0)+G(beta) = -1).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from gwsig_synth import make_crystal, make_inputs
+from gwsig_synth.group import rep_at_k, wigner_D_real
+from gwsig_synth.tensors import green_closed_form, tau_grid
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(fn):
+    with open(os.path.join(GOLD, fn)) as f:
+        return [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+
+
+# ---- P8: star finder against Table 2 -----------------------
+
+@pytest.mark.parametrize("row", _rows("table2_nik.txt"), ids=lambda r: r[0])
+def test_ibz_counts_match_table2(row):
+    name, expected = row[2], [int(v) for v in row[3:7]]
+    got = []
+    for n in (1, 2, 4, 6):
+        cr = make_crystal(name, mesh=(n, n, n))
+        got.append(len(cr.kmesh.stars(cr.sg)[0]))
+    assert got == expected      # only reproduced WITHOUT time reversal (A3)
+
+
+def test_table2_rotation_over_full_is_nik_over_nk():
+    """Rotation/Full = n_ik/N_k for AlP, GaAs, BN: cost is proportional
+    to the number of (k1 in IBZ, k2 in BZ) pairs.  Si's Full column is anomalous."""
+    for comp, nk, nik, full, rot, _ in _rows("table2_flops.txt"):
+        if comp == "Si" or int(nk) == 1:
+            continue
+        ratio = float(rot) / float(full)
+        assert abs(ratio - int(nik) / int(nk) ** 3) / ratio < 0.03
+
+
+@pytest.mark.parametrize("name,nops,ntrans,nik", [("cfg2", 48, 0, 10), ("cfg3", 48, 24, 16),
+                                                  ("cfg4", 12, 6, 28), ("cfg5", 48, 0, 29)])
+def test_config_groups(name, nops, ntrans, nik):
+    cr = make_crystal(name)
+    assert cr.sg.nops == nops
+    assert int((np.abs(cr.sg.w).max(axis=1) > 1e-9).sum()) == ntrans
+    assert len(cr.kmesh.stars(cr.sg)[0]) == nik
+    if name == "cfg3":      # Fd-3m: the fractional translation is (1/4,1/4,1/4) (BASELINE.json config 3)
+        w = cr.sg.w[np.abs(cr.sg.w).max(axis=1) > 1e-9]
+        assert np.allclose(w, 0.25)
+    if name == "cfg4":      # P6_3mc: screw/glide translation (0,0,1/2)
+        w = cr.sg.w[np.abs(cr.sg.w).max(axis=1) > 1e-9]
+        assert np.allclose(w, [0, 0, 0.5])
+    assert (cr.nao, cr.naux) == {"cfg2": (9, 18), "cfg3": (26, 116), "cfg4": (52, 232), "cfg5": (58, 300)}[name]
+
+
+# ---- P5: Wigner D and representation matrices -----------------------------------
+
+def test_wigner_D_properties():
+    cr = make_crystal("toy_wurtzite")
+    cr2 = make_crystal("toy_sc")
+    for sg in (cr.sg, cr2.sg):
+        R = sg.Rcart
+        for l in range(5):
+            D = [wigner_D_real(l, R[g]) for g in range(sg.nops)]
+            for g in range(sg.nops):
+                assert np.allclose(D[g] @ D[g].T, np.eye(2 * l + 1), atol=1e-12)
+                if l == 1:
+                    assert np.allclose(D[g], R[g], atol=1e-12)          # D^1 = R
+                if l == 0:
+                    assert np.allclose(D[g], 1.0)
+            # homomorphism on a few products
+            for g in (1, 5, sg.nops - 1):
+                for h in (2, 7):
+                    RR = R[g] @ R[h]
+                    assert np.allclose(wigner_D_real(l, RR), D[g] @ D[h], atol=1e-11)
+            # improper operations: D(-R) = (-1)^l D(R)
+            assert np.allclose(wigner_D_real(l, -R[3]), (-1) ** l * D[3], atol=1e-12)
+
+
+@pytest.mark.parametrize("name", ["toy_sc", "toy_diamond", "toy_wurtzite", "toy_rocksalt"])
+def test_rep_unitary_and_eq22_eq25_eq24a(name):
+    inp = make_inputs(name)
+    cr, sg, km = inp.cr, inp.cr.sg, inp.cr.kmesh
+    _, _, _, rot = km.stars(sg)
+    Wf = inp.W_full()
+    G = inp.G_full()
+    for g in range(sg.nops):
+        for k in range(km.nk):
+            kt = rot[g, k]
+            O = rep_at_k(cr.P_ao[g], cr.ao_atom, sg.shift[g], km.frac[kt])
+            Oa = rep_at_k(cr.P_aux[g], cr.aux_atom, sg.shift[g], km.frac[kt])
+            assert np.allclose(O @ O.conj().T, np.eye(cr.nao), atol=1e-12)
+            # Eq. 22 on H(k) and G(k,tau); Eq. 25 on W~
+            assert np.abs(inp.Hk[kt] - O @ inp.Hk[k] @ O.conj().T).max() < 1e-12
+            assert np.abs(G[kt] - O @ G[k] @ O.conj().T).max() < 1e-12
+            assert np.abs(Wf[kt] - Oa @ Wf[k] @ Oa.conj().T).max() < 1e-12
+    # Eq. 24a with the aux momentum q = k2 - k1, and the conj relation
+    for g in range(0, sg.nops, 5):
+        for (k1, k2) in [(0, 1), (1, 3), (5, 2), (7, 7)]:
+            k1t, k2t = rot[g, k1], rot[g, k2]
+            q = km.index(km.n[k2] - km.n[k1])
+            O1 = rep_at_k(cr.P_ao[g], cr.ao_atom, sg.shift[g], km.frac[k1t])
+            O2 = rep_at_k(cr.P_ao[g], cr.ao_atom, sg.shift[g], km.frac[k2t])
+            Oq = rep_at_k(cr.P_aux[g], cr.aux_atom, sg.shift[g], km.frac[rot[g, q]])
+            V = inp.V_pair(k1, k2)
+            pred = np.einsum("PQ,Ii,Qij,Jj->PIJ", Oq, O1, V, O2.conj(), optimize=True)
+            assert np.abs(pred - inp.V_pair(k1t, k2t)).max() < 1e-12
+            assert np.abs(inp.V_pair(k2, k1) - V.conj().transpose(0, 2, 1)).max() < 1e-13
+            assert np.abs(inp.V2_rows(k2, [k1])[0] - V).max() < 1e-13       # V2_rows(k1,[k2]) = V^{k2,k1}
+
+
+def test_W_hermitian_psd():
+    inp = make_inputs("toy_diamond")
+    Wf = inp.W_full()
+    assert np.abs(Wf - Wf.conj().transpose(0, 1, 3, 2)).max() < 1e-14
+    assert np.linalg.eigvalsh(Wf.reshape(-1, inp.naux, inp.naux)).min() > -1e-13
+
+
+# ---- P4: closed-form Green's function --------------------------------------------
+
+def test_green_two_level_analytic():
+    beta, e1, e2 = 7.0, -0.8, 1.3
+    tau = tau_grid(5, beta)
+    # H = R diag(e1,e2) R^T with a known rotation: G = -R diag(f) R^T, f = e^{-e tau}/(1+e^{-beta e})
+    c, s = np.cos(0.3), np.sin(0.3)
+    R = np.array([[c, -s], [s, c]])
+    G = green_closed_form(R @ np.diag([e1, e2]) @ R.T, 0.0, tau, beta)
+    for t, tt in enumerate(tau):
+        f = np.array([np.exp(-e * tt) / (1 + np.exp(-beta * e)) for e in (e1, e2)])
+        assert np.allclose(G[t], -R @ np.diag(f) @ R.T, atol=1e-14)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "toy_diamond"])
+def test_green_invariants(name):
+    inp = make_inputs(name)
+    G = inp.G_full()
+    n = inp.nao
+    assert np.abs(G[:, 0] + G[:, -1] + np.eye(n)).max() < 1e-12                 # G(0) + G(beta) = -1
+    assert np.abs(G - G.conj().transpose(0, 1, 3, 2)).max() < 1e-13            # Hermitian
+    assert np.linalg.eigvalsh(G.reshape(-1, n, n)).max() < 1e-14                # negative (semi)definite
+    nocc = 4 if name == "cfg1" else inp.cr.nocc
+    ne = np.mean([np.trace(-G[k, -1]).real for k in range(inp.nk)])             # N_e
+    assert abs(ne - nocc) < 0.2
+
+
+def test_green_large_beta_is_finite():
+    G = green_closed_form(np.diag([-3.0, 2.0]), 0.0, tau_grid(9, 200.0), 200.0)  # naive form overflows
+    assert np.isfinite(G).all()
+
+
+def test_cfg1_recipe():
+    inp = make_inputs("cfg1")
+    assert (inp.nk, inp.nao, inp.naux, inp.ntau, inp.beta) == (8, 8, 32, 16, 10.0)
+    V = inp.V_pair(2, 5)
+    assert np.abs(inp.V_pair(5, 2) - V.conj().transpose(0, 2, 1)).max() == 0
+    assert np.abs(inp.V_pair(3, 3) - inp.V_pair(3, 3).conj().transpose(0, 2, 1)).max() < 1e-15
+    assert abs(V.real.std() * np.sqrt(32) - 1) < 0.05 and abs(V.imag.std() * np.sqrt(32) - 1) < 0.05

@@ -1,0 +1,198 @@
+"""Pins for the CPU oracle: every test checks
+``oracle.sigma_oracle`` against something other than itself -- explicit loops,
+closed forms, or invariants that a dropped term / wrong sign / swapped index /
+transposed operand would break."""
+import numpy as np
+import pytest
+
+from gwsig_synth import make_inputs
+from gwsig_synth.group import rep_at_k
+from oracle.sigma_oracle import flops_per_output, sigma_brute, sigma_ref
+from paper_2405_09494_b200.symsetup import SymSetup
+
+
+def _c1(nao=3, naux=4, ntau=2, seed=5):
+    return make_inputs("cfg1", mesh=(2, 2, 2), nao=nao, naux=naux, ntau=ntau, beta=3.0, nocc=1, seed=seed)
+
+
+def _ref(inp, ks, G=None, W=None, V_pair=None):
+    G = inp.G_full() if G is None else G
+    W = inp.W_full() if W is None else W
+    V_pair = inp.V_pair if V_pair is None else V_pair
+    km = inp.kmesh
+    return sigma_ref(inp.nk, km.sub, lambda k: G[k], lambda q: W[q], V_pair, ks)
+
+
+# ---- P1: explicit seven-loop brute force ---------------------------------------
+
+def test_ref_equals_brute_force():
+    inp = _c1()
+    G, W = inp.G_full(), inp.W_full()
+    ks = [0, 3, 6]
+    b = sigma_brute(inp.nk, inp.kmesh.sub, G, W, inp.V_pair, ks)
+    r = _ref(inp, ks, G, W)
+    assert np.abs(b - r).max() < 1e-14 * max(1.0, np.abs(b).max())
+    assert np.abs(b).max() > 1e-3
+
+
+def test_ref_equals_brute_force_with_independent_V_partners():
+    """the oracle must not assume V^{k2,k1} = conj V^{k1,k2}: feed unrelated tensors."""
+    inp = _c1(seed=9)
+    rng = np.random.default_rng(3)
+    Vfree = rng.standard_normal((8, 8, 4, 3, 3)) + 1j * rng.standard_normal((8, 8, 4, 3, 3))
+    G = rng.standard_normal((8, 2, 3, 3)) + 1j * rng.standard_normal((8, 2, 3, 3))      # not Hermitian either
+    W = rng.standard_normal((8, 2, 4, 4)) + 1j * rng.standard_normal((8, 2, 4, 4))
+    vp = lambda a, b: Vfree[a, b]
+    b = sigma_brute(8, inp.kmesh.sub, G, W, vp, [1, 4])
+    r = sigma_ref(8, inp.kmesh.sub, lambda k: G[k], lambda q: W[q], vp, [1, 4])
+    assert np.abs(b - r).max() < 1e-12 * np.abs(b).max()
+
+
+# ---- P2: scalar closed forms ---------------------------------------------------------
+
+def test_scalar_closed_form():
+    """nao = naux = 1, k-independent v, g(tau), w(tau)  =>  Sigma = -|v|^2 g(tau) w(tau)."""
+    from gwsig_synth.group import KMesh
+    km = KMesh((2, 2, 2))
+    v = 0.7 - 0.4j
+    g = np.array([-0.9, -0.5, -0.2, -0.1])
+    w = np.array([0.3, 0.2, 0.25, 0.4])
+    G = np.broadcast_to(g[None, :, None, None], (8, 4, 1, 1))
+    W = np.broadcast_to(w[None, :, None, None], (8, 4, 1, 1))
+    vp = lambda k1, k2: np.full((1, 1, 1), v if k1 <= k2 else np.conj(v)) if k1 != k2 else np.full((1, 1, 1), abs(v))
+    # use |v| on the diagonal pairs (they must be Hermitian in ij) and v / conj(v) off-diagonal
+    out = sigma_ref(8, km.sub, lambda k: G[k], lambda q: W[q], vp, range(8))
+    assert np.allclose(out[:, :, 0, 0], -(abs(v) ** 2) * g * w, atol=1e-15)
+
+
+def test_exchange_like_closed_form():
+    """W~ = delta_{QQ'} w, G = g 1  =>  Sigma_ij = -(g w / Nk) sum_{q,Q,a} V^{k,k-q}_{Q,ia} V^{k-q,k}_{Q,aj}
+    (the shape of the exchange term Eq. 21c)."""
+    inp = _c1(nao=3, naux=4, ntau=2)
+    g, w = np.array([-0.6, -0.3]), np.array([0.5, 0.8])
+    G = np.einsum("t,ab->tab", g, np.eye(3))[None].repeat(8, 0)
+    W = np.einsum("t,ab->tab", w, np.eye(4))[None].repeat(8, 0)
+    out = _ref(inp, range(8), G, W)
+    for k in range(8):
+        acc = np.zeros((3, 3), complex)
+        for q in range(8):
+            kq = inp.kmesh.sub(k, q)
+            acc += np.einsum("Qia,Qaj->ij", inp.V_pair(k, kq), inp.V_pair(kq, k))
+        for t in range(2):
+            assert np.allclose(out[k, t], -(g[t] * w[t] / 8) * acc, atol=1e-13)
+
+
+def test_only_the_right_q_enters():
+    """G non-zero at one momentum p only, W~ non-zero at one q0 only: Sigma(k) is non-zero
+    only at k = p + q0 and equals the single term (pins the k-q bookkeeping and its sign)."""
+    inp = _c1()
+    G0, W0 = inp.G_full(), inp.W_full()
+    p, q0 = 5, 3
+    G = np.zeros_like(G0); G[p] = G0[p]
+    W = np.zeros_like(W0); W[q0] = W0[q0]
+    out = _ref(inp, range(8), G, W)
+    km = inp.kmesh
+    ktarget = int(km.index(km.n[p] + km.n[q0]))
+    for k in range(8):
+        if k != ktarget:
+            assert np.abs(out[k]).max() == 0
+    single = -np.einsum("Qia,tab,tQP,Pbj->tij", inp.V_pair(ktarget, p), G0[p], W0[q0], inp.V_pair(p, ktarget),
+                        optimize=True) / 8
+    assert np.allclose(out[ktarget], single, atol=1e-14)
+
+
+# ---- P3: bilinearity and gauge covariance ---------------------------------------------
+
+def test_bilinear_in_G_and_W():
+    inp = _c1()
+    i2 = _c1(seed=77)
+    G1, G2, W1, W2 = inp.G_full(), i2.G_full(), inp.W_full(), i2.W_full()
+    a, b = 0.3 - 1.1j, 2.0 + 0.5j
+    ks = [2, 7]
+    lhs = _ref(inp, ks, a * G1 + b * G2, W1)
+    assert np.allclose(lhs, a * _ref(inp, ks, G1, W1) + b * _ref(inp, ks, G2, W1), atol=1e-13)
+    lhs = _ref(inp, ks, G1, a * W1 + b * W2)
+    assert np.allclose(lhs, a * _ref(inp, ks, G1, W1) + b * _ref(inp, ks, G1, W2), atol=1e-13)
+
+
+def _rand_unitary(rng, n):
+    q, _ = np.linalg.qr(rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n)))
+    return q
+
+
+def test_gauge_covariance_orbital_and_aux():
+    """G -> T G T^dag, V^{k1k2} -> T^{k1} V T^{k2 dag}  =>  Sigma -> T Sigma T^dag; and in the aux space
+    V^{k1k2}_Q -> sum_P S^{q}_{QP} V_P with q = k2 - k1, W~^q -> S^q W~ S^{q dag}, with
+    S^{-q} = conj(S^q) (the relation J^{-q} = J^{q*} of PAPER.md:173 imposes on any aux basis change)
+    =>  Sigma unchanged.  This is exactly what block-basis parity relies on (Eq. 26-27)."""
+    inp = make_inputs("cfg1", mesh=(3, 2, 1), nao=3, naux=4, ntau=2, beta=3.0, nocc=1, seed=5)
+    km, nk = inp.kmesh, inp.nk
+    rng = np.random.default_rng(0)
+    T = [_rand_unitary(rng, inp.nao) for _ in range(nk)]
+    G, W = inp.G_full(), inp.W_full()
+    base = _ref(inp, range(nk), G, W)
+    Gt = np.stack([T[k] @ G[k] @ T[k].conj().T for k in range(nk)])
+    vt = lambda k1, k2: np.einsum("Ii,Qij,Jj->QIJ", T[k1], inp.V_pair(k1, k2), T[k2].conj())
+    out = _ref(inp, range(nk), Gt, W, vt)
+    for k in range(nk):
+        assert np.allclose(out[k], T[k] @ base[k] @ T[k].conj().T, atol=1e-13)
+
+    S = [None] * nk
+    for q in range(nk):
+        mq = int(km.index(-km.n[q]))
+        if S[q] is not None:
+            continue
+        if mq == q:
+            S[q] = np.linalg.qr(rng.standard_normal((inp.naux, inp.naux)))[0].astype(complex)
+        else:
+            S[q] = _rand_unitary(rng, inp.naux)
+            S[mq] = S[q].conj()
+    assert any(int(km.index(-km.n[q])) != q for q in range(nk))
+
+    def vs(k1, k2):
+        q = int(km.index(km.n[k2] - km.n[k1]))
+        return np.einsum("QP,Pij->Qij", S[q], inp.V_pair(k1, k2))
+
+    Wt = np.stack([S[q] @ W[q] @ S[q].conj().T for q in range(nk)])
+    out = _ref(inp, range(nk), G, Wt, vs)
+    assert np.allclose(out, base, atol=1e-13)
+    # and a wrong pairing (W~ transformed with the conjugate matrix) must NOT be invariant
+    Wbad = np.stack([S[q].conj() @ W[q] @ S[q].T for q in range(nk)])
+    assert np.abs(_ref(inp, range(nk), G, Wbad, vs) - base).max() > 1e-3 * np.abs(base).max()
+
+
+# ---- P7: symmetry invariants on oracle output ------------------------------------------
+
+@pytest.mark.parametrize("name", ["toy_diamond", "toy_wurtzite", "toy_sc"])
+def test_sigma_covariance_hermiticity_and_block_zeros(name):
+    inp = make_inputs(name)
+    cr, sg, km = inp.cr, inp.cr.sg, inp.cr.kmesh
+    S = _ref(inp, range(inp.nk))
+    scale = np.abs(S).max()
+    assert scale > 1e-4
+    # Hermiticity of Sigma_ij(k, tau)
+    assert np.abs(S - S.conj().transpose(0, 1, 3, 2)).max() < 1e-13 * scale
+    # Sigma(g k) = O Sigma(k) O^dagger  (Eq. 22)
+    _, _, _, rot = km.stars(sg)
+    for g in range(sg.nops):
+        for k in range(km.nk):
+            kt = rot[g, k]
+            O = rep_at_k(cr.P_ao[g], cr.ao_atom, sg.shift[g], km.frac[kt])
+            assert np.abs(S[kt] - O @ S[k] @ O.conj().T).max() < 1e-12 * scale
+    # exact zeros off the irrep blocks of U^dagger Sigma U  (Eq. 26)
+    st = SymSetup(cr.mesh, sg.W, sg.w, sg.shift, cr.P_ao, cr.P_aux, cr.ao_atom, cr.aux_atom)
+    ao = st.adapt("ao")
+    nontrivial = 0
+    for k in range(km.nk):
+        Sb = ao.U[k].conj().T @ S[k] @ ao.U[k]
+        mask = np.ones((cr.nao, cr.nao), bool)
+        for b in range(ao.nblk(k)):
+            mask[ao.off[k][b]:ao.off[k][b + 1], ao.off[k][b]:ao.off[k][b + 1]] = False
+        nontrivial += ao.nblk(k) > 1
+        if mask.any():
+            assert np.abs(Sb[:, mask]).max() < 1e-12 * scale
+    assert nontrivial > 0
+
+
+def test_flop_model():
+    assert flops_per_output(8, 8, 32) == 8 * 8 * (2 * 32 * 512 + 1024 * 64)

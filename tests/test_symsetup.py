@@ -1,0 +1,123 @@
+"""Host pre-step (Algorithm 1): Dirac characters, U^k, blocks,
+block-basis packing."""
+import numpy as np
+import pytest
+
+from gwsig_synth import make_crystal, make_inputs
+from paper_2405_09494_b200.symsetup import SymSetup
+
+
+def _setup(cr):
+    sg = cr.sg
+    return SymSetup(cr.mesh, sg.W, sg.w, sg.shift, cr.P_ao, cr.P_aux, cr.ao_atom, cr.aux_atom)
+
+
+def test_stars_agree_with_generator():
+    cr = make_crystal("toy_diamond4")
+    st = _setup(cr)
+    ir, ir_of, op_of, rot = cr.kmesh.stars(cr.sg)
+    assert np.array_equal(st.ir_list, ir) and np.array_equal(st.ir_of, ir_of) and np.array_equal(st.op_of, op_of)
+    assert np.array_equal(st.rot, rot)
+    for k in range(st.nk):       # op_of maps the representative onto k
+        assert st.rot[st.op_of[k], st.ir_of[k]] == k
+
+
+@pytest.mark.parametrize("name", ["toy_diamond", "toy_wurtzite"])
+def test_dirac_characters_commute_with_all_D(name):
+    """'all Dirac characters commute with the representation of all group elements
+    and with each other' -- for the projective representation D^k of Eq. 7 at non-symmorphic k too."""
+    cr = make_crystal(name)
+    st = _setup(cr)
+    for k in st.ir_list:
+        lg = st.little_group(int(k))
+        Om = st.dirac_characters("ao", int(k))
+        Ds = [st.D("ao", int(k), g) for g in lg]
+        for O1 in Om:
+            for D in Ds:
+                assert np.abs(O1 @ D - D @ O1).max() < 1e-12
+            for O2 in Om:
+                assert np.abs(O1 @ O2 - O2 @ O1).max() < 1e-12
+        # projective composition law Eq. 5 with the factor system of Eq. 8 is at least a phase
+        for a in range(len(lg)):
+            for b in range(len(lg)):
+                Pab = Ds[a] @ Ds[b]
+                hits = [np.abs(Pab - (Pab.ravel()[np.argmax(np.abs(Dc))] / Dc.ravel()[np.argmax(np.abs(Dc))]) * Dc).max()
+                        for Dc in Ds]
+                assert min(hits) < 1e-11
+
+
+def test_block_sizes_diamond_sp():
+    """Gamma of diamond s+p: isotypic blocks 1,1,3,3; X: 2,4,2 (as multisets {2,2,4}); L: 2,2,2,2."""
+    cr = make_crystal("toy_diamond")
+    st = _setup(cr)
+    ao = st.adapt("ao")
+    sizes = {tuple(int(v) for v in st.n[k]): sorted(ao.sizes(k).tolist()) for k in range(st.nk)}
+    assert sizes[(0, 0, 0)] == [1, 1, 3, 3]
+    # 2x2x2 fcc mesh: Gamma, 4 L points (one index = 1 ... ), 3 X points
+    got = sorted(map(tuple, (sizes[k] for k in sizes)))
+    assert got.count((1, 1, 3, 3)) == 1
+    assert got.count((2, 2, 4)) == 3          # X star
+    assert got.count((2, 2, 2, 2)) == 4       # L star
+
+
+@pytest.mark.parametrize("name", ["toy_diamond", "toy_wurtzite", "toy_rocksalt"])
+def test_U_unitary_and_inputs_block_diagonal(name):
+    inp = make_inputs(name)
+    cr = inp.cr
+    st = _setup(cr)
+    ao, aux = st.adapt("ao"), st.adapt("aux")
+    G, W = inp.G_full(), inp.W_full()
+    for k in range(st.nk):
+        assert np.abs(ao.U[k].conj().T @ ao.U[k] - np.eye(cr.nao)).max() < 1e-12
+        assert np.array_equal(ao.off[k], ao.off[st.ir_of[k]])
+        pk = st.pack_diag_blocks(G[k], ao.U[k], ao.off[k])           # raises if not block diagonal
+        back = ao.U[k] @ st.unpack_diag_blocks(pk, ao.off[k]) @ ao.U[k].conj().T
+        assert np.abs(back - G[k]).max() < 1e-12
+        pw = st.pack_diag_blocks(W[k], aux.U[k], aux.off[k])
+        # S5 gauge: the packed block-basis data of a star member equals that of its representative
+        kI = st.ir_of[k]
+        assert np.abs(pk - st.pack_diag_blocks(G[kI], ao.U[kI], ao.off[kI])).max() < 1e-12
+        assert np.abs(pw - st.pack_diag_blocks(W[kI], aux.U[kI], aux.off[kI])).max() < 1e-12
+
+
+def test_block_V2_roundtrip_and_selection():
+    inp = make_inputs("toy_diamond")
+    st = _setup(inp.cr)
+    ao, aux = st.adapt("ao"), st.adapt("aux")
+    nall = nallowed = 0
+    for k1 in st.ir_list:
+        for k2 in range(st.nk):
+            V2 = inp.V2_rows(int(k1), [k2])[0]
+            tr, packed = st.block_V2(V2, int(k1), k2, ao, aux)
+            q = st.sub(int(k1), k2)
+            nall += aux.nblk(q) * ao.nblk(k2) * ao.nblk(int(k1))
+            nallowed += len(tr)
+            # energy conservation: the allowed blocks carry all of V
+            assert abs(np.linalg.norm(packed) - np.linalg.norm(V2)) < 1e-12 * np.linalg.norm(V2)
+            # explicit triples reproduce the same packing
+            tr2, packed2 = st.block_V2(V2, int(k1), k2, ao, aux, triples=tr)
+            assert np.array_equal(packed, packed2)
+    assert 0 < nallowed < nall
+
+
+def test_executed_mac_ratio_is_in_the_papers_range():
+    """soft shape check against Table 2's Si rows: block/rotation = 0.22 (2^3), 0.40 (4^3)."""
+    for name, lo, hi in [("toy_diamond", 0.1, 0.45), ("toy_diamond4", 0.25, 0.65)]:
+        inp = make_inputs(name)
+        st = _setup(inp.cr)
+        ao, aux = st.adapt("ao"), st.adapt("aux")
+        nao, naux = inp.nao, inp.naux
+        dense = blk = 0.0
+        for k1 in st.ir_list:
+            V2s = inp.V2_rows(int(k1), range(st.nk))
+            for k2 in range(st.nk):
+                q = st.sub(int(k1), k2)
+                tr, _ = st.block_V2(V2s[k2], int(k1), k2, ao, aux)
+                sp, s2, s1 = aux.sizes(q), ao.sizes(k2), ao.sizes(int(k1))
+                dense += 2 * naux * nao ** 3 + naux ** 2 * nao ** 2
+                for p in range(len(sp)):
+                    Np = sum(s2[a] * s1[i] for (pp, a, i) in tr if pp == p)
+                    blk += sp[p] ** 2 * Np
+                for (p, a, i) in tr:
+                    blk += sp[p] * s1[i] * s2[a] ** 2 + sp[p] * s2[a] * s1[i] ** 2
+        assert lo < blk / dense < hi, (name, blk / dense)
