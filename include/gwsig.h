@@ -1,0 +1,161 @@
+/* gwsig -- C-ABI boundary of the B200-native GW self-energy evaluation.
+ *
+ * The operation (Eq. 16 of arXiv 2405.09494, readings A1/A6/A7 of DESIGN.md):
+ *
+ *   Sigma_ij(k,tau) = -(1/Nk) sum_{q in BZ} sum_{QQ'ab}
+ *        conj(V2[Q,a,i]) * G_ab(k-q,tau) * W_{QQ'}(q,tau) * V2[Q',b,j],      V2 = V^{k-q,k}
+ *
+ * evaluated for k in the irreducible wedge, optionally in the
+ * Dirac-character block basis over the symmetry-allowed blocks only,
+ * following the pair loop of Algorithm 4.  W is the paper's P^q(tau) (Eq. 19).
+ *
+ * Conventions
+ *   - every function returns 0 on success, a negative gwsig_status otherwise; nothing is
+ *     launched on error; gwsig_last_error() returns a static description of the last failure.
+ *   - all array arguments are CALLER-OWNED; the library copies what it keeps at the call.
+ *   - "host" / "dev" in a comment says where the pointer must live.  Complex numbers are
+ *     interleaved (re, im) doubles (complex128).  Matrices are row-major.
+ *   - momenta are mesh indices  k = (n0*N1 + n1)*N2 + n2,  k - q is taken modulo the mesh.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - no CPU fallback exists: without a CUDA device sigma_* return GWSIG_ERR_CUDA.
+ *     The plan-side calls (set_*, get_ibz, pair_*, plan_*) are host-only and need no device.
+ */
+#ifndef GWSIG_H
+#define GWSIG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gwsig_ctx gwsig_ctx;
+
+typedef enum {
+  GWSIG_OK = 0,
+  GWSIG_ERR_ARG = -1,      /* bad size / NULL pointer / call order                               */
+  GWSIG_ERR_SYMMETRY = -2, /* rotation does not map the mesh onto itself, D not orthogonal, ...   */
+  GWSIG_ERR_BLOCKS = -3,   /* block maps do not tile [0,n), star members disagree, bad triples    */
+  GWSIG_ERR_CUDA = -4,     /* CUDA runtime error (message holds cudaGetErrorString)               */
+  GWSIG_ERR_ORDER = -5     /* pushed pair range out of order / incomplete at sigma_end            */
+} gwsig_status;
+
+typedef enum {
+  GWSIG_FULL_BZ = 0,   /* k1 over the whole mesh, G and W given on the whole mesh, no unfold      */
+  GWSIG_IBZ = 1,       /* k1 over the wedge; G, W given at wedge points, unfolded by Eq. 22 / 25  */
+  GWSIG_IBZ_BLOCK = 2  /* wedge + block basis: packed irrep blocks, allowed triples only          */
+} gwsig_mode;
+
+typedef enum {
+  GWSIG_ENGINE_DMMA = 0,     /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA)       */
+  GWSIG_ENGINE_REFERENCE = 1 /* one-thread-per-element DFMA kernels on the same plan (debug)      */
+} gwsig_engine;
+
+/* ---- life cycle ------------------------------------------------------------------------ */
+/* device >= 0: CUDA device ordinal used by sigma_*; device < 0: host-only context (plan calls). */
+int gwsig_create(gwsig_ctx** out, int device);
+int gwsig_destroy(gwsig_ctx* ctx);
+const char* gwsig_last_error(const gwsig_ctx* ctx);
+
+/* ---- problem statement ----------------------------------------------------------------------
+ * set_lattice: a[9] rows = primitive vectors (host); mesh[3] = Gamma-centred k mesh;
+ * nao, naux = orbital / auxiliary basis sizes; ntau = number of imaginary-time points (Sigma is
+ * pointwise in tau, the grid itself is not needed); beta is recorded only.                        */
+int gwsig_set_lattice(gwsig_ctx* ctx, const double a[9], const int mesh[3], int nao, int naux, int ntau,
+                      double beta);
+
+/* set_atoms: natom; pos[natom*3] fractional (host, recorded); ao_atom[nao], aux_atom[naux] = atom
+ * each basis function sits on (needed for the per-atom phase of Eq. 3).           */
+int gwsig_set_atoms(gwsig_ctx* ctx, int natom, const double* pos, const int* ao_atom, const int* aux_atom);
+
+/* set_symmetry (all host):
+ *   rot[nops*9]   integer rotation W in lattice coordinates, r -> W r + w        ({alpha|v})
+ *   trans[nops*3] fractional translation w (recorded; enters D^k of Eq. 7 only, i.e. the pre-step)
+ *   D_ao[nops*nao*nao], D_aux[nops*naux*naux]  k-independent REAL representation
+ *                 (atom permutation (x) real Wigner D, Eq. 3-4); row index = image function
+ *   shift[nops*natom*3] integer lattice shift s_x with  W tau_x + w = tau_perm(x) + s_x ("translation
+ *                 vector between rotated and original atom").  The library multiplies the
+ *                 phase exp(-2 pi i k~ . s_x) into column (x,m) itself:  O^k = D . diag(phase)  (Eq. 3)
+ *   mode          gwsig_mode.   nops = 0 is allowed only with GWSIG_FULL_BZ.
+ * Builds the k maps, the stars (representative = first member in index order, op_of = first
+ * operation in input order mapping it there; space-group operations only, no time reversal) and
+ * the (q-major) pair list.  Errors: GWSIG_ERR_SYMMETRY.                                            */
+int gwsig_set_symmetry(gwsig_ctx* ctx, int nops, const int* rot, const double* trans, const double* D_ao,
+                       const double* D_aux, const int* shift, int mode);
+
+/* set_blocks (IBZ_BLOCK only, host): irrep (isotypic) block maps per mesh point in CSR form:
+ *   nblk_ao[Nk], ao_block_off[sum(nblk_ao)+Nk] : for each k the nblk+1 offsets 0 = o_0 < ... = nao
+ *   nblk_aux[Nk], aux_block_off[...]           : same for the auxiliary basis at q
+ *   U_ao [Nk*nao*nao], U_aux[Nk*naux*naux]     : symmetry-adapted bases U^k (Eq. 26) or NULL.
+ *       NULL  = the gauge U^{k'} = O^{k_I}(alpha^) U^{k_I} for star members, for which O_block of
+ *               Eq. 28 is the identity and block data of k' are those of its representative;
+ *       given = the library forms O_block = U^{k' dagger} O^{k_I}(alpha^) U^{k_I} (Eq. 28) for
+ *               op_of[k'] and unfolds packed blocks with it (must come out block diagonal).
+ * Errors: GWSIG_ERR_BLOCKS (offsets do not tile, star member's block sizes differ from its
+ * representative's, O_block not block diagonal).                                                   */
+int gwsig_set_blocks(gwsig_ctx* ctx, const int* nblk_ao, const int* ao_block_off, const int* nblk_aux,
+                     const int* aux_block_off, const double* U_ao, const double* U_aux);
+
+/* set_triples (IBZ_BLOCK only, host): symmetry-allowed blocks of V2 for every pair ("only non-zero
+ * blocks are considered").  triple_ptr[npairs+1] CSR; triples[3*nt] = (p, alpha, iota):
+ * aux block of q, orbital block of k2, orbital block of k1; sorted by p within a pair.              */
+int gwsig_set_triples(gwsig_ctx* ctx, int64_t npairs, const int64_t* triple_ptr, const int32_t* triples);
+
+/* ---- what the plan decided (host outputs; any pointer may be NULL) --------------------------- */
+int gwsig_get_ibz(gwsig_ctx* ctx, int* nik, int* ir_list /*[nik]*/, int* ir_of /*[Nk]*/, int* op_of /*[Nk]*/);
+/* pairs are ordered q-major: pair = q * nk1 + i1, k1 = out_list[i1], k2 = k1 - q                   */
+int gwsig_pair_count(gwsig_ctx* ctx, int64_t* npairs, int* nk1);
+int gwsig_pair_info(gwsig_ctx* ctx, int64_t pair, int* k1, int* k2, int* q, int64_t* v_offset /*elements*/,
+                    int64_t* v_elems);
+/* element counts / offsets of the G, W and Sigma buffers sigma_eval expects in the current mode:
+ *   FULL_BZ : G[Nk][ntau][nao][nao], W[Nk][ntau][naux][naux], Sigma[Nk][ntau][nao][nao]
+ *   IBZ     : the same with the wedge points (in ir_list order) instead of Nk
+ *   IBZ_BLOCK: per wedge point [ntau][sum_b n_b^2] packed diagonal blocks, points concatenated     */
+int gwsig_buffer_sizes(gwsig_ctx* ctx, int64_t* g_elems, int64_t* w_elems, int64_t* sigma_elems, int64_t* v_elems);
+
+/* ---- the evaluation -------------------------------------------------------------------------
+ * sigma_begin : dG, dW (dev, layouts above), dSigma (dev, written by sigma_end).  Unfolds G to the
+ *               full zone (Eq. 22 / 28), zeroes the accumulator.
+ * sigma_push_pairs : dV (dev) holds V2 = V^{k2,k1}_{Q,bj} for pairs p0 .. p0+np-1, packed back to
+ *               back in pair order ([naux][nao][nao] dense; allowed blocks in IBZ_BLOCK mode, see
+ *               DESIGN.md).  Ranges must be pushed in increasing order without gaps and should
+ *               cover whole q (multiples of nk1) for best reuse of the unfolded W(q).  Runs
+ *               X = V G, Y = W X, Sigma += Y V  (Algorithm 4 lines 5-8) for those pairs, all tau.
+ *               Exists because V does not fit on the device at the large configs.
+ * sigma_end   : epilogue  Sigma = -(1/Nk) * accumulated (optionally Hermitised) -> dSigma.
+ * sigma_eval  : begin + one push of all pairs + end.
+ * All work is enqueued on `stream`; results are valid after the stream is synchronised.           */
+int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSigma, void* stream);
+int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV);
+int gwsig_sigma_end(gwsig_ctx* ctx);
+int gwsig_sigma_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, const void* dW, void* dSigma, void* stream);
+
+/* ---- options and accounting ------------------------------------------------------------------ */
+/* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
+ * default 4096), "tau_chunk" (0 = from the budget)                                                */
+int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value);
+/* real flops (8 per complex multiply-add) of one evaluation: the full-BZ dense equivalent
+ * Nk^2 ntau 8(2A+B) and what the current mode's plan actually asks for.
+ * In IBZ_BLOCK mode `executed` needs set_triples first.                                            */
+int gwsig_flop_counts(gwsig_ctx* ctx, double* full_bz_equiv, double* executed);
+/* number of kernel launches and DMMA-engine device time bookkeeping of the last evaluation         */
+int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
+
+/* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
+ * stage: 1 = X = V G, 2 = Y = W X, 3 = Sigma += Y V, 4 = unfold step 1, 5 = unfold step 2.
+ * Descriptors are the structs of include/gwsig_plan.h; offsets are in complex elements relative
+ * to the operand bases documented there.                                                           */
+int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, int64_t* nproblems, int64_t* nsegs,
+                      int64_t* ntiles);
+int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, void* problems_out, void* segs_out);
+
+/* ---- FP64 peak probe (measurement support; needs a device) -------------------------------------
+ * kind 0: register-only mma.sync.m8n8k4.f64 issue-rate loop; kind 1: register-only DFMA loop.
+ * Returns achieved TFLOP/s over `iters` inner iterations on every SM (CUDA-event timed).           */
+int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters,
+                     double* tflops, double* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWSIG_H */

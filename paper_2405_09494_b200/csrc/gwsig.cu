@@ -1,0 +1,589 @@
+// C-ABI of the gwsig library (include/gwsig.h): context, device buffers, launch orchestration.
+// Order of work per evaluation:
+//   sigma_begin : [a1] unfold G to the full zone (IBZ mode)            -> Gbz
+//   sigma_push  : [a2] unfold W for the q of the pushed pairs (IBZ)    -> W ring
+//                 per sub-batch of whole q's, per tau chunk:
+//                 [a3] X = conj(V2)^T G, [a4] Y = W^T X, [a5] Sigma_acc += Y V2   (grouped GEMM engine)
+//   sigma_end   : [a6] Sigma = -(1/Nk) Sigma_acc (optional Hermitise)
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "gwsig.h"
+#include "kernels_aux.cuh"
+#include "plan.hpp"
+#include "zgemm_grouped.cuh"
+
+using gwsig::cplx;
+using gwsig::Plan;
+using gwsig::StagePlan;
+
+namespace {
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  cudaError_t ensure(size_t need) {
+    if (need <= bytes) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr; bytes = 0;
+    cudaError_t e = cudaMalloc(&p, need);
+    if (e == cudaSuccess) bytes = need;
+    return e;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+};
+
+struct DevStage {
+  DevBuf prob, seg;
+  int nprob = 0;
+  long long ntiles = 0;
+  int shape_class = 0;
+};
+struct DevPlan { DevStage st[3]; };
+
+}  // namespace
+
+struct gwsig_ctx {
+  Plan plan;
+  int device = -1;
+  bool cuda_ready = false;
+  int num_sms = 0;
+  std::string err;
+  // options
+  int engine = GWSIG_ENGINE_DMMA;
+  int hermitize = 0;
+  long long scratch_mib = 8192;
+  int tau_chunk = 0;
+  // evaluation state
+  bool in_eval = false;
+  const double2* dG = nullptr;
+  const double2* dW = nullptr;
+  double2* dSigma = nullptr;
+  cudaStream_t stream = nullptr;
+  long long next_pair = 0;
+  long long launches = 0;
+  // device buffers
+  DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
+  DevBuf tgt_src, tgt_op, colphase_ao, ell_cols_ao, ell_vals_ao, ell_cnt_ao;     // unfold tables (ao)
+  DevBuf wtgt_src, wtgt_op, colphase_aux, ell_cols_aux, ell_vals_aux, ell_cnt_aux;
+  int maxnz_ao = 0, maxnz_aux = 0;
+  bool tables_ready = false;
+  int n_epidesc = 0;
+  std::map<std::tuple<long long, long long, int, int>, std::unique_ptr<DevPlan>> plan_cache;
+  int counter_slot = 0;
+  static constexpr int kCounterSlots = 8192;
+};
+
+namespace {
+
+int fail(gwsig_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+int cuda_fail(gwsig_ctx* c, cudaError_t e, const char* where) {
+  return fail(c, GWSIG_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                                   \
+  do {                                                             \
+    cudaError_t e__ = (call);                                      \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);     \
+  } while (0)
+
+int ensure_cuda(gwsig_ctx* ctx) {
+  if (ctx->cuda_ready) return GWSIG_OK;
+  if (ctx->device < 0) return fail(ctx, GWSIG_ERR_CUDA, "host-only context (device < 0): no CUDA device; there is no CPU fallback");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= ctx->device)
+    return fail(ctx, GWSIG_ERR_CUDA, std::string("no usable CUDA device (there is no CPU fallback): ") + cudaGetErrorString(e));
+  CU(cudaSetDevice(ctx->device));
+  CU(cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, ctx->device));
+  ctx->cuda_ready = true;
+  return GWSIG_OK;
+}
+
+template <class T>
+int upload(gwsig_ctx* ctx, DevBuf& b, const std::vector<T>& v) {
+  size_t bytes = std::max<size_t>(v.size() * sizeof(T), 16);
+  CU(b.ensure(bytes));
+  if (!v.empty()) CU(cudaMemcpyAsync(b.p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
+  // the host vector may be a temporary: make the copy complete before returning
+  CU(cudaStreamSynchronize(ctx->stream));
+  return GWSIG_OK;
+}
+
+// ELL form of the real representation matrices (non-zeros per row <= 2l+1)
+void build_ell(const std::vector<double>& D, int nops, int n, std::vector<int>& cols, std::vector<double>& vals,
+               std::vector<int>& cnt, int& maxnz) {
+  maxnz = 1;
+  cnt.assign((size_t)nops * n, 0);
+  for (int g = 0; g < nops; ++g)
+    for (int r = 0; r < n; ++r) {
+      int c = 0;
+      for (int j = 0; j < n; ++j)
+        if (std::fabs(D[((size_t)g * n + r) * n + j]) > 1e-13) ++c;
+      cnt[(size_t)g * n + r] = c;
+      maxnz = std::max(maxnz, c);
+    }
+  cols.assign((size_t)nops * n * maxnz, 0);
+  vals.assign((size_t)nops * n * maxnz, 0.0);
+  for (int g = 0; g < nops; ++g)
+    for (int r = 0; r < n; ++r) {
+      int c = 0;
+      for (int j = 0; j < n; ++j) {
+        double v = D[((size_t)g * n + r) * n + j];
+        if (std::fabs(v) > 1e-13) {
+          cols[((size_t)g * n + r) * maxnz + c] = j;
+          vals[((size_t)g * n + r) * maxnz + c] = v;
+          ++c;
+        }
+      }
+    }
+}
+
+// exp(-2 pi i k' . s_atom(c)(g)) for target k' reached with operation g   (Eq. 3)
+void column_phases(const Plan& P, const std::vector<int>& targets, const std::vector<int>& atom_of, int n,
+                   std::vector<double2>& out) {
+  out.resize(targets.size() * (size_t)n);
+  for (size_t t = 0; t < targets.size(); ++t) {
+    int k = targets[t], g = P.op_of[k], nn[3];
+    P.kcoords(k, nn);
+    for (int c = 0; c < n; ++c) {
+      const int* s = &P.shift[((size_t)g * P.natom + atom_of[c]) * 3];
+      double ph = -2.0 * M_PI * ((double)nn[0] * s[0] / P.N[0] + (double)nn[1] * s[1] / P.N[1] + (double)nn[2] * s[2] / P.N[2]);
+      out[t * n + c] = make_double2(std::cos(ph), std::sin(ph));
+    }
+  }
+}
+
+int prepare_tables(gwsig_ctx* ctx) {
+  if (ctx->tables_ready) return GWSIG_OK;
+  const Plan& P = ctx->plan;
+  if (P.mode == GWSIG_IBZ) {
+    std::vector<int> cols, cnt;
+    std::vector<double> vals;
+    build_ell(P.D_ao, P.nops, P.nao, cols, vals, cnt, ctx->maxnz_ao);
+    int rc;
+    if ((rc = upload(ctx, ctx->ell_cols_ao, cols))) return rc;
+    if ((rc = upload(ctx, ctx->ell_vals_ao, vals))) return rc;
+    if ((rc = upload(ctx, ctx->ell_cnt_ao, cnt))) return rc;
+    build_ell(P.D_aux, P.nops, P.naux, cols, vals, cnt, ctx->maxnz_aux);
+    if ((rc = upload(ctx, ctx->ell_cols_aux, cols))) return rc;
+    if ((rc = upload(ctx, ctx->ell_vals_aux, vals))) return rc;
+    if ((rc = upload(ctx, ctx->ell_cnt_aux, cnt))) return rc;
+    std::vector<int> targets(P.nk), src(P.nk), op(P.nk);
+    for (int k = 0; k < P.nk; ++k) { targets[k] = k; src[k] = P.ir_index[P.ir_of[k]]; op[k] = P.op_of[k]; }
+    std::vector<double2> ph;
+    column_phases(P, targets, P.ao_atom, P.nao, ph);
+    if ((rc = upload(ctx, ctx->colphase_ao, ph))) return rc;
+    column_phases(P, targets, P.aux_atom, P.naux, ph);
+    if ((rc = upload(ctx, ctx->colphase_aux, ph))) return rc;
+    if ((rc = upload(ctx, ctx->tgt_src, src))) return rc;
+    if ((rc = upload(ctx, ctx->tgt_op, op))) return rc;
+  }
+  // epilogue descriptors: one batch of ntau square matrices per (output k, block)
+  std::vector<EpiDesc> ed;
+  for (int i = 0; i < P.nk1; ++i) {
+    const std::vector<int>& off = P.ao_off[P.out_list[i]];
+    long long stride = P.mode == GWSIG_IBZ_BLOCK ? gwsig::sumsq(off) : (long long)P.nao * P.nao;
+    long long o = P.sig_off[i];
+    for (size_t b = 0; b + 1 < off.size(); ++b) {
+      int n = off[b + 1] - off[b];
+      ed.push_back(EpiDesc{o, stride, n, P.ntau});
+      o += (long long)n * n;
+    }
+  }
+  ctx->n_epidesc = (int)ed.size();
+  int rc = upload(ctx, ctx->epidesc, ed);
+  if (rc) return rc;
+  ctx->tables_ready = true;
+  return GWSIG_OK;
+}
+
+int get_dev_plan(gwsig_ctx* ctx, long long p0, long long np, int nt, int q_first, DevPlan** out) {
+  auto key = std::make_tuple(p0, np, nt, q_first);
+  auto it = ctx->plan_cache.find(key);
+  if (it != ctx->plan_cache.end()) { *out = it->second.get(); return GWSIG_OK; }
+  std::unique_ptr<DevPlan> dp(new DevPlan());
+  for (int s = 0; s < 3; ++s) {
+    StagePlan sp;
+    int rc = ctx->plan.build_stage(p0, np, nt, s + 1, q_first, sp);
+    if (rc) return fail(ctx, rc, "internal: build_stage failed");
+    DevStage& d = dp->st[s];
+    d.nprob = (int)sp.prob.size();
+    d.ntiles = sp.ntiles;
+    d.shape_class = sp.shape_class;
+    if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
+    if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
+  }
+  *out = dp.get();
+  ctx->plan_cache[key] = std::move(dp);
+  return GWSIG_OK;
+}
+
+int run_stage(gwsig_ctx* ctx, const DevStage& d, const double2* A, const double2* B, double2* C, int t0) {
+  if (d.ntiles <= 0) return GWSIG_OK;
+  if (ctx->counter_slot >= gwsig_ctx::kCounterSlots) {
+    CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
+    ctx->counter_slot = 0;
+  }
+  ZgParams zp;
+  zp.A = A; zp.B = B; zp.C = C;
+  zp.prob = (const gwsig_problem*)d.prob.p;
+  zp.seg = (const gwsig_seg*)d.seg.p;
+  zp.nprob = d.nprob;
+  zp.total_tiles = d.ntiles;
+  zp.t0 = t0;
+  zp.counter = (unsigned long long*)ctx->counters.p + ctx->counter_slot++;
+  CU(zg_launch(ctx->engine, d.shape_class, zp, ctx->num_sms, ctx->stream));
+  ctx->launches++;
+  return GWSIG_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+int gwsig_create(gwsig_ctx** out, int device) {
+  if (!out) return GWSIG_ERR_ARG;
+  *out = new gwsig_ctx();
+  (*out)->device = device;
+  return GWSIG_OK;
+}
+
+int gwsig_destroy(gwsig_ctx* ctx) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  if (ctx->cuda_ready) {
+    cudaSetDevice(ctx->device);
+    DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
+                      &ctx->probe_sink, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
+                      &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux};
+    for (DevBuf* b : bufs) b->release();
+    for (auto& kv : ctx->plan_cache)
+      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); }
+  }
+  delete ctx;
+  return GWSIG_OK;
+}
+
+const char* gwsig_last_error(const gwsig_ctx* ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+
+static void invalidate(gwsig_ctx* ctx) {
+  ctx->tables_ready = false;
+  for (auto& kv : ctx->plan_cache)
+    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); }
+  ctx->plan_cache.clear();
+  ctx->in_eval = false;
+}
+
+int gwsig_set_lattice(gwsig_ctx* ctx, const double a[9], const int mesh[3], int nao, int naux, int ntau, double beta) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  int rc = ctx->plan.set_lattice(a, mesh, nao, naux, ntau, beta);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
+int gwsig_set_atoms(gwsig_ctx* ctx, int natom, const double* pos, const int* ao_atom, const int* aux_atom) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  int rc = ctx->plan.set_atoms(natom, pos, ao_atom, aux_atom);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
+int gwsig_set_symmetry(gwsig_ctx* ctx, int nops, const int* rot, const double* trans, const double* D_ao,
+                       const double* D_aux, const int* shift, int mode) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  int rc = ctx->plan.set_symmetry(nops, rot, trans, D_ao, D_aux, shift, mode);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
+int gwsig_set_blocks(gwsig_ctx* ctx, const int* nblk_ao, const int* ao_block_off, const int* nblk_aux,
+                     const int* aux_block_off, const double* U_ao, const double* U_aux) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  if (U_ao || U_aux)
+    return fail(ctx, GWSIG_ERR_ARG, "set_blocks: explicit U (general gauge, Eq. 28 unfold) is not available yet; pass NULL "
+                                    "and use the gauge U^{k'} = O^{k_I}(alpha) U^{k_I}");
+  int rc = ctx->plan.set_blocks(nblk_ao, ao_block_off, nblk_aux, aux_block_off, U_ao, U_aux);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
+int gwsig_set_triples(gwsig_ctx* ctx, int64_t npairs, const int64_t* triple_ptr, const int32_t* triples) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  int rc = ctx->plan.set_triples(npairs, triple_ptr, triples);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
+int gwsig_get_ibz(gwsig_ctx* ctx, int* nik, int* ir_list, int* ir_of, int* op_of) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  const Plan& P = ctx->plan;
+  if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "get_ibz: call set_symmetry first");
+  if (nik) *nik = (int)P.ir_list.size();
+  if (ir_list) std::copy(P.ir_list.begin(), P.ir_list.end(), ir_list);
+  if (ir_of) std::copy(P.ir_of.begin(), P.ir_of.end(), ir_of);
+  if (op_of) std::copy(P.op_of.begin(), P.op_of.end(), op_of);
+  return GWSIG_OK;
+}
+
+int gwsig_pair_count(gwsig_ctx* ctx, int64_t* npairs, int* nk1) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  if (!ctx->plan.have_sym) return fail(ctx, GWSIG_ERR_ARG, "pair_count: call set_symmetry first");
+  if (npairs) *npairs = ctx->plan.npairs;
+  if (nk1) *nk1 = ctx->plan.nk1;
+  return GWSIG_OK;
+}
+
+int gwsig_pair_info(gwsig_ctx* ctx, int64_t pair, int* k1, int* k2, int* q, int64_t* v_offset, int64_t* v_elems) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  const Plan& P = ctx->plan;
+  if (!P.have_sym || pair < 0 || pair >= P.npairs) return fail(ctx, GWSIG_ERR_ARG, "pair_info: bad pair index or no symmetry set");
+  int a, b, c, d;
+  P.pair(pair, a, b, c, d);
+  if (k1) *k1 = a;
+  if (k2) *k2 = b;
+  if (q) *q = c;
+  if (v_offset || v_elems) {
+    if (P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "pair_info: V layout needs set_triples in IBZ_BLOCK mode");
+    if (v_offset) *v_offset = P.v_off[pair];
+    if (v_elems) *v_elems = P.v_off[pair + 1] - P.v_off[pair];
+  }
+  return GWSIG_OK;
+}
+
+int gwsig_buffer_sizes(gwsig_ctx* ctx, int64_t* g_elems, int64_t* w_elems, int64_t* sigma_elems, int64_t* v_elems) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  const Plan& P = ctx->plan;
+  if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "buffer_sizes: call set_symmetry first");
+  if (g_elems) *g_elems = P.g_elems;
+  if (w_elems) *w_elems = P.w_elems;
+  if (sigma_elems) *sigma_elems = P.sig_elems;
+  if (v_elems) *v_elems = P.v_off.empty() ? -1 : P.v_off.back();
+  return GWSIG_OK;
+}
+
+int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
+  if (!ctx || !key) return GWSIG_ERR_ARG;
+  std::string k(key);
+  if (k == "engine") {
+    if (value != GWSIG_ENGINE_DMMA && value != GWSIG_ENGINE_REFERENCE) return fail(ctx, GWSIG_ERR_ARG, "set_option: bad engine");
+    ctx->engine = (int)value;
+  } else if (k == "hermitize") ctx->hermitize = value != 0;
+  else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
+  else if (k == "tau_chunk") { if (value < 0) return fail(ctx, GWSIG_ERR_ARG, "set_option: tau_chunk < 0"); ctx->tau_chunk = (int)value; }
+  else return fail(ctx, GWSIG_ERR_ARG, "set_option: unknown key " + k);
+  return GWSIG_OK;
+}
+
+int gwsig_flop_counts(gwsig_ctx* ctx, double* full_bz_equiv, double* executed) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  if (!ctx->plan.have_sym) return fail(ctx, GWSIG_ERR_ARG, "flop_counts: call set_symmetry first");
+  double f, e;
+  ctx->plan.flop_counts(f, e);
+  if (full_bz_equiv) *full_bz_equiv = f;
+  if (executed) *executed = e;
+  return GWSIG_OK;
+}
+
+int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches) {
+  if (!ctx || !launches) return GWSIG_ERR_ARG;
+  *launches = ctx->launches;
+  return GWSIG_OK;
+}
+
+int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, int64_t* nproblems, int64_t* nsegs,
+                      int64_t* ntiles) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  const Plan& P = ctx->plan;
+  if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
+  StagePlan sp;
+  int rc = P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
+  if (rc) return fail(ctx, rc, "plan_counts: bad range / stage");
+  if (nproblems) *nproblems = (int64_t)sp.prob.size();
+  if (nsegs) *nsegs = (int64_t)sp.seg.size();
+  if (ntiles) *ntiles = sp.ntiles;
+  return GWSIG_OK;
+}
+
+int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, void* problems_out, void* segs_out) {
+  if (!ctx || !problems_out || !segs_out) return GWSIG_ERR_ARG;
+  const Plan& P = ctx->plan;
+  if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
+  StagePlan sp;
+  int rc = P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
+  if (rc) return fail(ctx, rc, "plan_get: bad range / stage");
+  std::memcpy(problems_out, sp.prob.data(), sp.prob.size() * sizeof(gwsig_problem));
+  std::memcpy(segs_out, sp.seg.data(), sp.seg.size() * sizeof(gwsig_seg));
+  return GWSIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSigma, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: call set_symmetry first");
+  if (P.mode == GWSIG_IBZ_BLOCK && (!P.have_blocks || !P.have_triples))
+    return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: IBZ_BLOCK mode needs set_blocks and set_triples");
+  if (!dG || !dW || !dSigma) return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: NULL device pointer");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)stream;
+  ctx->dG = (const double2*)dG;
+  ctx->dW = (const double2*)dW;
+  ctx->dSigma = (double2*)dSigma;
+  if ((rc = prepare_tables(ctx))) return rc;
+  CU(ctx->sigacc.ensure(std::max<size_t>(P.sig_elems * sizeof(double2), 16)));
+  CU(cudaMemsetAsync(ctx->sigacc.p, 0, P.sig_elems * sizeof(double2), ctx->stream));
+  CU(ctx->counters.ensure(gwsig_ctx::kCounterSlots * sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
+  ctx->counter_slot = 0;
+  ctx->launches = 0;
+  if (P.mode == GWSIG_IBZ) {
+    // [a1] G(k') = O G(k_I) O^dagger for every mesh point (Eq. 22; Algorithm 2 step 2)
+    CU(ctx->gbz.ensure((size_t)P.nk * P.ntau * P.nao * P.nao * sizeof(double2)));
+    UnfoldParams up;
+    up.src = ctx->dG; up.dst = (double2*)ctx->gbz.p;
+    up.tgt_src = (const int*)ctx->tgt_src.p; up.tgt_op = (const int*)ctx->tgt_op.p;
+    up.colphase = (const double2*)ctx->colphase_ao.p;
+    up.ell_cols = (const int*)ctx->ell_cols_ao.p; up.ell_vals = (const double*)ctx->ell_vals_ao.p;
+    up.ell_cnt = (const int*)ctx->ell_cnt_ao.p;
+    up.n = P.nao; up.ntau = P.ntau; up.maxnz = ctx->maxnz_ao;
+    CU(launch_unfold_sparse(up, P.nk, ctx->stream));
+    ctx->launches++;
+  }
+  ctx->next_pair = 0;
+  ctx->in_eval = true;
+  return GWSIG_OK;
+}
+
+int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!ctx->in_eval) return fail(ctx, GWSIG_ERR_ORDER, "sigma_push_pairs: call sigma_begin first");
+  if (np < 1 || p0 != ctx->next_pair || p0 + np > P.npairs)
+    return fail(ctx, GWSIG_ERR_ORDER, "sigma_push_pairs: ranges must be pushed in increasing order without gaps");
+  if (!dV) return fail(ctx, GWSIG_ERR_ARG, "sigma_push_pairs: NULL device pointer");
+  CU(cudaSetDevice(ctx->device));
+  const double2* Vbase = (const double2*)dV;
+  const int nk1 = P.nk1;
+  const int q_first = (int)(p0 / nk1), q_last = (int)((p0 + np - 1) / nk1);
+
+  // [a2] unfold W for the q of this push (Eq. 25; Algorithm 4 line 6)
+  const double2* Wsrc = ctx->dW;
+  if (P.mode == GWSIG_IBZ) {
+    const int nq = q_last - q_first + 1;
+    CU(ctx->wring.ensure((size_t)nq * P.ntau * P.naux * P.naux * sizeof(double2)));
+    UnfoldParams up;
+    up.src = ctx->dW; up.dst = (double2*)ctx->wring.p;
+    up.tgt_src = (const int*)ctx->tgt_src.p + q_first; up.tgt_op = (const int*)ctx->tgt_op.p + q_first;
+    up.colphase = (const double2*)ctx->colphase_aux.p + (size_t)q_first * P.naux;
+    up.ell_cols = (const int*)ctx->ell_cols_aux.p; up.ell_vals = (const double*)ctx->ell_vals_aux.p;
+    up.ell_cnt = (const int*)ctx->ell_cnt_aux.p;
+    up.n = P.naux; up.ntau = P.ntau; up.maxnz = ctx->maxnz_aux;
+    CU(launch_unfold_sparse(up, nq, ctx->stream));
+    ctx->launches++;
+    Wsrc = (const double2*)ctx->wring.p;
+  }
+  const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
+
+  // sub-batches of pairs (whole q's where possible) and tau chunks sized to the scratch budget
+  const double budget = (double)ctx->scratch_mib * 1048576.0 / (2.0 * sizeof(double2));   // elements of X (= of Y)
+  long long s0 = p0;
+  while (s0 < p0 + np) {
+    // grow the sub-batch by whole q's while X for all tau still fits
+    long long s1 = std::min<long long>(p0 + np, (s0 / nk1 + 1) * nk1);
+    while (s1 < p0 + np) {
+      long long s2 = std::min<long long>(p0 + np, s1 + nk1);
+      if ((double)(P.v_off[s2] - P.v_off[s0]) * P.ntau > budget) break;
+      s1 = s2;
+    }
+    const long long ns = s1 - s0;
+    const double per_tau = (double)(P.v_off[s1] - P.v_off[s0]);
+    int nt_max = ctx->tau_chunk > 0 ? ctx->tau_chunk : (int)std::max(1.0, std::floor(budget / std::max(per_tau, 1.0)));
+    nt_max = std::min(nt_max, P.ntau);
+    const int nchunks = (P.ntau + nt_max - 1) / nt_max;
+    const int nt = (P.ntau + nchunks - 1) / nchunks;
+    const size_t xbytes = (size_t)std::max(per_tau * nt, 1.0) * sizeof(double2);
+    CU(ctx->xbuf.ensure(xbytes));
+    CU(ctx->ybuf.ensure(xbytes));
+    const double2* Vsub = Vbase + (P.v_off[s0] - P.v_off[p0]);
+    for (int t0 = 0; t0 < P.ntau; t0 += nt) {
+      const int ntc = std::min(nt, P.ntau - t0);
+      DevPlan* dp = nullptr;
+      int rc = get_dev_plan(ctx, s0, ns, ntc, q_first, &dp);
+      if (rc) return rc;
+      if ((rc = run_stage(ctx, dp->st[0], Vsub, Gsrc, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
+      if ((rc = run_stage(ctx, dp->st[1], Wsrc, (const double2*)ctx->xbuf.p, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
+      if ((rc = run_stage(ctx, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
+    }
+    s0 = s1;
+  }
+  ctx->next_pair = p0 + np;
+  return GWSIG_OK;
+}
+
+int gwsig_sigma_end(gwsig_ctx* ctx) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!ctx->in_eval) return fail(ctx, GWSIG_ERR_ORDER, "sigma_end: call sigma_begin first");
+  if (ctx->next_pair != P.npairs) return fail(ctx, GWSIG_ERR_ORDER, "sigma_end: not all pairs were pushed");
+  CU(cudaSetDevice(ctx->device));
+  // [a6] Sigma = -(1/Nk) sum_q Sigma^{k,q}   (Eq. 16 prefactor)
+  EpilogueParams ep;
+  ep.acc = (const double2*)ctx->sigacc.p;
+  ep.out = ctx->dSigma;
+  ep.desc = (const EpiDesc*)ctx->epidesc.p;
+  ep.scale = -1.0 / (double)P.nk;
+  ep.hermitize = ctx->hermitize;
+  CU(launch_epilogue(ep, ctx->n_epidesc, ctx->num_sms, ctx->stream));
+  ctx->launches++;
+  ctx->in_eval = false;
+  return GWSIG_OK;
+}
+
+int gwsig_sigma_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, const void* dW, void* dSigma, void* stream) {
+  int rc = gwsig_sigma_begin(ctx, dG, dW, dSigma, stream);
+  if (rc) return rc;
+  rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
+  if (rc) return rc;
+  return gwsig_sigma_end(ctx);
+}
+
+int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters, double* tflops,
+                     double* ms) {
+  if (!ctx || !tflops || warps_per_block < 1 || warps_per_block > 32 || blocks_per_sm < 1 || iters < 1) return GWSIG_ERR_ARG;
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  CU(ctx->probe_sink.ensure(64));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  double flops = 0;
+  CU(launch_probe(kind, warps_per_block, ctx->num_sms * blocks_per_sm, iters / 8 + 1, (double*)ctx->probe_sink.p, nullptr, &flops));  // warm-up
+  CU(cudaEventRecord(e0, nullptr));
+  CU(launch_probe(kind, warps_per_block, ctx->num_sms * blocks_per_sm, iters, (double*)ctx->probe_sink.p, nullptr, &flops));
+  CU(cudaEventRecord(e1, nullptr));
+  CU(cudaEventSynchronize(e1));
+  float t = 0;
+  CU(cudaEventElapsedTime(&t, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *tflops = flops / (t * 1e-3) / 1e12;
+  if (ms) *ms = t;
+  return GWSIG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,134 @@
+// HBM-bound helper kernels of the hot path: structured unfold (Eq. 22 / 25), the Sigma
+// epilogue (scale, optional Hermitise), and the FP64 issue-rate probes used by bench.py.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "kernels_aux.cuh"
+
+namespace {
+
+// out[r,c] = sum_{m in nz(r)} sum_{n in nz(c)} P[r,m] ph[m] X[m,n] P[c,n] conj(ph[n])
+// O^k(alpha^) = P . diag(ph) is never formed densely: P = (atom permutation) x (real Wigner D) has at
+// most 2l+1 <= 9 entries per row (Eq. 3-4).  X^{k~} = O X^k O^dagger (Eq. 22).
+__global__ void __launch_bounds__(256) unfold_sparse_kernel(UnfoldParams p) {
+  const int tgt = blockIdx.y / p.ntau, t = blockIdx.y % p.ntau;
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n = p.n;
+  if (e >= n * n) return;
+  const int r = e / n, c = e - r * n;
+  const int op = p.tgt_op[tgt];
+  const double2* X = p.src + ((long long)p.tgt_src[tgt] * p.ntau + t) * n * n;
+  const double2* ph = p.colphase + (long long)tgt * n;
+  const int* rc = p.ell_cols + ((long long)op * n + r) * p.maxnz;
+  const double* rv = p.ell_vals + ((long long)op * n + r) * p.maxnz;
+  const int* cc = p.ell_cols + ((long long)op * n + c) * p.maxnz;
+  const double* cv = p.ell_vals + ((long long)op * n + c) * p.maxnz;
+  const int nr = p.ell_cnt[op * n + r], nc = p.ell_cnt[op * n + c];
+  double sr = 0.0, si = 0.0;
+  for (int a = 0; a < nr; ++a) {
+    const int m = rc[a];
+    const double2 pm = ph[m];
+    const double wr = rv[a] * pm.x, wi = rv[a] * pm.y;        // P[r,m] ph[m]
+    double tr = 0.0, ti = 0.0;                                // sum_n X[m,n] P[c,n] conj(ph[n])
+    for (int b = 0; b < nc; ++b) {
+      const int nn = cc[b];
+      const double2 x = X[(long long)m * n + nn];
+      const double2 pn = ph[nn];
+      const double ur = cv[b] * pn.x, ui = -cv[b] * pn.y;
+      tr += x.x * ur - x.y * ui;
+      ti += x.x * ui + x.y * ur;
+    }
+    sr += wr * tr - wi * ti;
+    si += wr * ti + wi * tr;
+  }
+  p.dst[((long long)tgt * p.ntau + t) * n * n + e] = make_double2(sr, si);
+}
+
+// Sigma = scale * acc, optionally (Sigma + Sigma^dagger)/2, for a list of square-matrix batches.
+__global__ void __launch_bounds__(256) epilogue_kernel(EpilogueParams p) {
+  const int d = blockIdx.y;
+  const EpiDesc D = p.desc[d];
+  const long long total = (long long)D.count * D.n * D.n;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int nn = D.n * D.n;
+    const long long t = e / nn;
+    const int ij = (int)(e - t * nn);
+    const int i = ij / D.n, j = ij - i * D.n;
+    const long long base = D.off + t * D.stride;
+    double2 v = p.acc[base + ij];
+    if (p.hermitize) {
+      const double2 w = p.acc[base + (long long)j * D.n + i];
+      v.x = 0.5 * (v.x + w.x);
+      v.y = 0.5 * (v.y - w.y);
+    }
+    p.out[base + ij] = make_double2(p.scale * v.x, p.scale * v.y);
+  }
+}
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+// register-only issue-rate probes: NACC independent accumulator chains per warp
+template <int NACC>
+__global__ void probe_dmma_kernel(long long iters, double* sink) {
+  double c0[NACC], c1[NACC];
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) { c0[a] = threadIdx.x * 1e-9; c1[a] = a * 1e-9; }
+  double x = 1.0 + 1e-12 * threadIdx.x, y = 1.0 - 1e-12 * threadIdx.x;
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) dmma884(c0[a], c1[a], x, y);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) s += c0[a] + c1[a];
+  if (s == 123.456) sink[0] = s;
+}
+
+template <int NACC>
+__global__ void probe_dfma_kernel(long long iters, double* sink) {
+  double c[NACC];
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) c[a] = threadIdx.x * 1e-9 + a;
+  double x = 1.0 + 1e-12 * threadIdx.x, y = 1e-9;
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) c[a] = fma(c[a], x, y);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) s += c[a];
+  if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace
+
+cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream) {
+  if (ntarget <= 0) return cudaSuccess;
+  dim3 grid((unsigned)((p.n * p.n + 255) / 256), (unsigned)(ntarget * p.ntau));
+  unfold_sparse_kernel<<<grid, 256, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_epilogue(const EpilogueParams& p, int ndesc, int num_sms, cudaStream_t stream) {
+  if (ndesc <= 0) return cudaSuccess;
+  dim3 grid((unsigned)(num_sms > 0 ? 4 : 1), (unsigned)ndesc);
+  epilogue_kernel<<<grid, 256, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long iters, double* sink, cudaStream_t stream,
+                         double* flops_out) {
+  constexpr int NACC = 16;
+  if (kind == 0) {
+    probe_dmma_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
+    *flops_out = (double)blocks * warps_per_block * (double)iters * NACC * 512.0;       // 8*8*4*2 per DMMA
+  } else {
+    probe_dfma_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
+    *flops_out = (double)blocks * warps_per_block * 32.0 * (double)iters * NACC * 2.0;
+  }
+  return cudaGetLastError();
+}

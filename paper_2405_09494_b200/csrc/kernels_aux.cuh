@@ -1,0 +1,35 @@
+// Declarations of the helper kernels (unfold, epilogue, FP64 probes).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+struct UnfoldParams {
+  const double2* src;       // [nsrc][ntau][n][n]   wedge data
+  double2* dst;             // [ntarget][ntau][n][n]
+  const int* tgt_src;       // [ntarget] wedge index of the star representative
+  const int* tgt_op;        // [ntarget] operation alpha with alpha k_I = k'
+  const double2* colphase;  // [ntarget][n]  exp(-2 pi i k' . s_atom(c))   (Eq. 3)
+  const int* ell_cols;      // [nops][n][maxnz]  non-zeros of the real representation matrix
+  const double* ell_vals;   // [nops][n][maxnz]
+  const int* ell_cnt;       // [nops][n]
+  int n, ntau, maxnz;
+};
+
+struct EpiDesc {
+  long long off;     // first element of the batch
+  long long stride;  // elements between consecutive matrices (tau)
+  int n, count;      // n x n matrices, `count` of them
+};
+
+struct EpilogueParams {
+  const double2* acc;
+  double2* out;
+  const EpiDesc* desc;  // device
+  double scale;
+  int hermitize;
+};
+
+cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream);
+cudaError_t launch_epilogue(const EpilogueParams& p, int ndesc, int num_sms, cudaStream_t stream);
+cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long iters, double* sink, cudaStream_t stream,
+                         double* flops_out);

@@ -1,0 +1,490 @@
+// Host plan (step a0): see plan.hpp.  Citations are PAPER.md lines of arXiv 2405.09494.
+#include "plan.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "zgemm_grouped.cuh"
+
+namespace gwsig {
+
+int Plan::kindex(int n0, int n1, int n2) const {
+  auto md = [](int v, int m) { int r = v % m; return r < 0 ? r + m : r; };
+  return (md(n0, N[0]) * N[1] + md(n1, N[1])) * N[2] + md(n2, N[2]);
+}
+void Plan::kcoords(int k, int n[3]) const {
+  n[2] = k % N[2];
+  n[1] = (k / N[2]) % N[1];
+  n[0] = k / (N[1] * N[2]);
+}
+int Plan::ksub(int k, int q) const {
+  int a_[3], b_[3];
+  kcoords(k, a_);
+  kcoords(q, b_);
+  return kindex(a_[0] - b_[0], a_[1] - b_[1], a_[2] - b_[2]);
+}
+
+int Plan::set_lattice(const double a_[9], const int mesh[3], int nao_, int naux_, int ntau_, double beta_) {
+  if (!a_ || !mesh) { err = "set_lattice: NULL argument"; return GWSIG_ERR_ARG; }
+  if (mesh[0] < 1 || mesh[1] < 1 || mesh[2] < 1 || nao_ < 1 || naux_ < 1 || ntau_ < 1) {
+    err = "set_lattice: mesh, nao, naux and ntau must be positive"; return GWSIG_ERR_ARG;
+  }
+  if ((long long)mesh[0] * mesh[1] * mesh[2] > (1 << 20)) { err = "set_lattice: mesh too large"; return GWSIG_ERR_ARG; }
+  std::memcpy(a, a_, sizeof(a));
+  for (int i = 0; i < 3; ++i) N[i] = mesh[i];
+  nk = mesh[0] * mesh[1] * mesh[2];
+  nao = nao_; naux = naux_; ntau = ntau_; beta = beta_;
+  have_lattice = true;
+  have_atoms = have_sym = have_blocks = have_triples = false;
+  return GWSIG_OK;
+}
+
+int Plan::set_atoms(int natom_, const double* pos_, const int* ao_atom_, const int* aux_atom_) {
+  if (!have_lattice) { err = "set_atoms: call set_lattice first"; return GWSIG_ERR_ARG; }
+  if (natom_ < 1 || !pos_ || !ao_atom_ || !aux_atom_) { err = "set_atoms: bad argument"; return GWSIG_ERR_ARG; }
+  for (int i = 0; i < nao; ++i)
+    if (ao_atom_[i] < 0 || ao_atom_[i] >= natom_) { err = "set_atoms: ao_atom out of range"; return GWSIG_ERR_ARG; }
+  for (int i = 0; i < naux; ++i)
+    if (aux_atom_[i] < 0 || aux_atom_[i] >= natom_) { err = "set_atoms: aux_atom out of range"; return GWSIG_ERR_ARG; }
+  natom = natom_;
+  pos.assign(pos_, pos_ + 3 * natom_);
+  ao_atom.assign(ao_atom_, ao_atom_ + nao);
+  aux_atom.assign(aux_atom_, aux_atom_ + naux);
+  have_atoms = true;
+  have_sym = have_blocks = have_triples = false;
+  return GWSIG_OK;
+}
+
+static bool int_inverse(const int* W, int* Winv) {
+  long long d = (long long)W[0] * (W[4] * W[8] - W[5] * W[7]) - (long long)W[1] * (W[3] * W[8] - W[5] * W[6]) +
+                (long long)W[2] * (W[3] * W[7] - W[4] * W[6]);
+  if (d != 1 && d != -1) return false;
+  int c[9] = {W[4] * W[8] - W[5] * W[7], W[2] * W[7] - W[1] * W[8], W[1] * W[5] - W[2] * W[4],
+              W[5] * W[6] - W[3] * W[8], W[0] * W[8] - W[2] * W[6], W[2] * W[3] - W[0] * W[5],
+              W[3] * W[7] - W[4] * W[6], W[1] * W[6] - W[0] * W[7], W[0] * W[4] - W[1] * W[3]};
+  for (int i = 0; i < 9; ++i) Winv[i] = (int)(c[i] * d);
+  return true;
+}
+
+static bool orthogonal(const double* D, int n) {
+  for (int i = 0; i < n; ++i)
+    for (int j = i; j < n; ++j) {
+      double s = 0;
+      for (int k = 0; k < n; ++k) s += D[(size_t)i * n + k] * D[(size_t)j * n + k];
+      if (std::fabs(s - (i == j ? 1.0 : 0.0)) > 1e-8) return false;
+    }
+  return true;
+}
+
+int Plan::set_symmetry(int nops_, const int* rot_, const double* trans_, const double* D_ao_, const double* D_aux_,
+                       const int* shift_, int mode_) {
+  if (!have_lattice) { err = "set_symmetry: call set_lattice first"; return GWSIG_ERR_ARG; }
+  if (mode_ != GWSIG_FULL_BZ && mode_ != GWSIG_IBZ && mode_ != GWSIG_IBZ_BLOCK) { err = "set_symmetry: bad mode"; return GWSIG_ERR_ARG; }
+  if (nops_ < 0 || (nops_ == 0 && mode_ != GWSIG_FULL_BZ)) { err = "set_symmetry: nops = 0 needs GWSIG_FULL_BZ"; return GWSIG_ERR_ARG; }
+  if (nops_ > 0 && (!rot_ || !trans_ || !D_ao_ || !D_aux_ || !shift_ || !have_atoms)) {
+    err = "set_symmetry: NULL argument or set_atoms not called"; return GWSIG_ERR_ARG;
+  }
+  mode = mode_;
+  if (nops_ == 0) {            // no symmetry: identity only
+    nops = 1;
+    rot = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+    trans = {0, 0, 0};
+    if (!have_atoms) { natom = 1; ao_atom.assign(nao, 0); aux_atom.assign(naux, 0); pos = {0, 0, 0}; have_atoms = true; }
+    shift.assign((size_t)3 * natom, 0);
+    D_ao.assign((size_t)nao * nao, 0.0);
+    for (int i = 0; i < nao; ++i) D_ao[(size_t)i * nao + i] = 1.0;
+    D_aux.assign((size_t)naux * naux, 0.0);
+    for (int i = 0; i < naux; ++i) D_aux[(size_t)i * naux + i] = 1.0;
+  } else {
+    nops = nops_;
+    rot.assign(rot_, rot_ + 9 * (size_t)nops);
+    trans.assign(trans_, trans_ + 3 * (size_t)nops);
+    D_ao.assign(D_ao_, D_ao_ + (size_t)nops * nao * nao);
+    D_aux.assign(D_aux_, D_aux_ + (size_t)nops * naux * naux);
+    shift.assign(shift_, shift_ + (size_t)nops * natom * 3);
+    for (int g = 0; g < nops; ++g) {
+      if (!orthogonal(&D_ao[(size_t)g * nao * nao], nao) || !orthogonal(&D_aux[(size_t)g * naux * naux], naux)) {
+        err = "set_symmetry: representation matrix of operation " + std::to_string(g) + " is not orthogonal";
+        return GWSIG_ERR_SYMMETRY;
+      }
+    }
+  }
+  // k~ = k W^-1 (row vector) on mesh indices; must stay on the mesh
+  rotk.assign((size_t)nops * nk, 0);
+  for (int g = 0; g < nops; ++g) {
+    int Winv[9];
+    if (!int_inverse(&rot[9 * g], Winv)) { err = "set_symmetry: rotation " + std::to_string(g) + " is not unimodular"; return GWSIG_ERR_SYMMETRY; }
+    for (int k = 0; k < nk; ++k) {
+      int n[3], out[3];
+      kcoords(k, n);
+      for (int j = 0; j < 3; ++j) {
+        long long acc = 0;
+        for (int i = 0; i < 3; ++i) {
+          long long t = (long long)n[i] * Winv[3 * i + j] * N[j];
+          if (t % N[i] != 0) { err = "set_symmetry: rotation " + std::to_string(g) + " does not map the k mesh onto itself"; return GWSIG_ERR_SYMMETRY; }
+          acc += t / N[i];
+        }
+        long long r = acc % N[j];
+        out[j] = (int)(r < 0 ? r + N[j] : r);
+      }
+      rotk[(size_t)g * nk + k] = kindex(out[0], out[1], out[2]);
+    }
+    // a rotation must permute the mesh
+    std::vector<char> seen(nk, 0);
+    for (int k = 0; k < nk; ++k) seen[rotk[(size_t)g * nk + k]] = 1;
+    for (int k = 0; k < nk; ++k)
+      if (!seen[k]) { err = "set_symmetry: rotation " + std::to_string(g) + " is not a permutation of the mesh"; return GWSIG_ERR_SYMMETRY; }
+  }
+  // stars: representative = first member in index order; op_of = first op mapping it there
+  ir_of.assign(nk, -1); op_of.assign(nk, -1); ir_index.assign(nk, -1); ir_list.clear();
+  for (int k = 0; k < nk; ++k) {
+    if (ir_of[k] >= 0) continue;
+    ir_index[k] = (int)ir_list.size();
+    ir_list.push_back(k);
+    for (int g = 0; g < nops; ++g) {
+      int kp = rotk[(size_t)g * nk + k];
+      if (ir_of[kp] < 0) { ir_of[kp] = k; op_of[kp] = g; }
+    }
+  }
+  if (op_of[ir_list[0]] != 0 && nops > 0) {
+    // the first operation must be the identity for op_of[representative] to be the identity
+    for (int k : ir_list)
+      if (rotk[(size_t)op_of[k] * nk + k] != k) { err = "set_symmetry: internal star error"; return GWSIG_ERR_SYMMETRY; }
+  }
+  out_list.clear();
+  if (mode == GWSIG_FULL_BZ) { out_list.resize(nk); std::iota(out_list.begin(), out_list.end(), 0); }
+  else out_list = ir_list;
+  nk1 = (int)out_list.size();
+  npairs = (long long)nk * nk1;
+  // trivial (one-block) maps; set_blocks overrides them in IBZ_BLOCK mode
+  ao_off.assign(nk, std::vector<int>{0, nao});
+  aux_off.assign(nk, std::vector<int>{0, naux});
+  U_ao.clear(); U_aux.clear(); general_gauge = false;
+  have_sym = true;
+  have_blocks = have_triples = false;
+  triple_ptr.clear(); triples.clear();
+  return finalize_layouts();
+}
+
+int Plan::set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nblk_aux, const int* aux_block_off,
+                     const double* U_ao_, const double* U_aux_) {
+  if (!have_sym || mode != GWSIG_IBZ_BLOCK) { err = "set_blocks: needs set_symmetry with GWSIG_IBZ_BLOCK"; return GWSIG_ERR_ARG; }
+  if (!nblk_ao || !ao_block_off || !nblk_aux || !aux_block_off) { err = "set_blocks: NULL argument"; return GWSIG_ERR_ARG; }
+  if ((U_ao_ == nullptr) != (U_aux_ == nullptr)) { err = "set_blocks: give both U_ao and U_aux or neither"; return GWSIG_ERR_ARG; }
+  auto read = [&](const int* nblk, const int* offs, int n, std::vector<std::vector<int>>& out, const char* what) -> int {
+    out.assign(nk, {});
+    size_t pos_ = 0;
+    for (int k = 0; k < nk; ++k) {
+      if (nblk[k] < 1 || nblk[k] > n) { err = std::string("set_blocks: bad block count (") + what + ")"; return GWSIG_ERR_BLOCKS; }
+      out[k].assign(offs + pos_, offs + pos_ + nblk[k] + 1);
+      pos_ += nblk[k] + 1;
+      if (out[k].front() != 0 || out[k].back() != n) { err = std::string("set_blocks: blocks do not tile [0,n) (") + what + ")"; return GWSIG_ERR_BLOCKS; }
+      for (size_t b = 0; b + 1 < out[k].size(); ++b)
+        if (out[k][b + 1] <= out[k][b]) { err = std::string("set_blocks: block offsets not increasing (") + what + ")"; return GWSIG_ERR_BLOCKS; }
+    }
+    for (int k = 0; k < nk; ++k)
+      if (out[k] != out[ir_of[k]]) { err = std::string("set_blocks: star member's blocks differ from its representative's (") + what + ")"; return GWSIG_ERR_BLOCKS; }
+    return GWSIG_OK;
+  };
+  int rc = read(nblk_ao, ao_block_off, nao, ao_off, "ao");
+  if (rc) return rc;
+  rc = read(nblk_aux, aux_block_off, naux, aux_off, "aux");
+  if (rc) return rc;
+  general_gauge = U_ao_ != nullptr;
+  if (general_gauge) {
+    const cplx* ua = reinterpret_cast<const cplx*>(U_ao_);
+    const cplx* ux = reinterpret_cast<const cplx*>(U_aux_);
+    U_ao.assign(ua, ua + (size_t)nk * nao * nao);
+    U_aux.assign(ux, ux + (size_t)nk * naux * naux);
+  } else { U_ao.clear(); U_aux.clear(); }
+  have_blocks = true;
+  have_triples = false;
+  triple_ptr.clear(); triples.clear();
+  return finalize_layouts();
+}
+
+int Plan::set_triples(int64_t npairs_, const int64_t* triple_ptr_, const int32_t* triples_) {
+  if (!have_blocks || mode != GWSIG_IBZ_BLOCK) { err = "set_triples: needs set_blocks in GWSIG_IBZ_BLOCK mode"; return GWSIG_ERR_ARG; }
+  if (npairs_ != npairs || !triple_ptr_ || (!triples_ && triple_ptr_[npairs_] > 0)) { err = "set_triples: wrong pair count or NULL argument"; return GWSIG_ERR_ARG; }
+  if (triple_ptr_[0] != 0) { err = "set_triples: triple_ptr[0] must be 0"; return GWSIG_ERR_BLOCKS; }
+  for (long long p = 0; p < npairs; ++p) {
+    if (triple_ptr_[p + 1] < triple_ptr_[p]) { err = "set_triples: triple_ptr not monotone"; return GWSIG_ERR_BLOCKS; }
+    int k1, k2, q, i1;
+    pair(p, k1, k2, q, i1);
+    int prev = -1;
+    for (long long t = triple_ptr_[p]; t < triple_ptr_[p + 1]; ++t) {
+      const int32_t* T = triples_ + 3 * t;
+      if (T[0] < 0 || T[0] >= (int)aux_off[q].size() - 1 || T[1] < 0 || T[1] >= (int)ao_off[k2].size() - 1 || T[2] < 0 ||
+          T[2] >= (int)ao_off[k1].size() - 1) { err = "set_triples: block index out of range at pair " + std::to_string(p); return GWSIG_ERR_BLOCKS; }
+      if (T[0] < prev) { err = "set_triples: triples of a pair must be sorted by aux block"; return GWSIG_ERR_BLOCKS; }
+      prev = T[0];
+    }
+  }
+  triple_ptr.assign(triple_ptr_, triple_ptr_ + npairs + 1);
+  triples.assign(triples_, triples_ + 3 * triple_ptr_[npairs]);
+  have_triples = true;
+  return finalize_layouts();
+}
+
+int Plan::finalize_layouts() {
+  const bool blk = mode == GWSIG_IBZ_BLOCK;
+  // input G / W: per wedge point (IBZ modes) or per mesh point (FULL_BZ), packed blocks in block mode
+  const std::vector<int>& pts = mode == GWSIG_FULL_BZ ? out_list : ir_list;
+  g_in_off.assign(pts.size() + 1, 0);
+  w_in_off.assign(pts.size() + 1, 0);
+  for (size_t i = 0; i < pts.size(); ++i) {
+    long long gs = blk ? sumsq(ao_off[pts[i]]) : (long long)nao * nao;
+    long long ws = blk ? sumsq(aux_off[pts[i]]) : (long long)naux * naux;
+    g_in_off[i + 1] = g_in_off[i] + gs * ntau;
+    w_in_off[i + 1] = w_in_off[i] + ws * ntau;
+  }
+  g_elems = g_in_off.back();
+  w_elems = w_in_off.back();
+  sig_off.assign(nk1 + 1, 0);
+  for (int i = 0; i < nk1; ++i)
+    sig_off[i + 1] = sig_off[i] + (blk ? sumsq(ao_off[out_list[i]]) : (long long)nao * nao) * ntau;
+  sig_elems = sig_off.back();
+  v_off.clear();
+  if (!blk) {
+    v_off.resize(npairs + 1);
+    for (long long p = 0; p <= npairs; ++p) v_off[p] = p * (long long)naux * nao * nao;
+  } else if (have_triples) {
+    v_off.assign(npairs + 1, 0);
+    for (long long p = 0; p < npairs; ++p) {
+      int k1, k2, q, i1;
+      pair(p, k1, k2, q, i1);
+      long long s = 0;
+      for (long long t = triple_ptr[p]; t < triple_ptr[p + 1]; ++t) {
+        const int32_t* T = &triples[3 * t];
+        s += (long long)(aux_off[q][T[0] + 1] - aux_off[q][T[0]]) * (ao_off[k2][T[1] + 1] - ao_off[k2][T[1]]) *
+             (ao_off[k1][T[2] + 1] - ao_off[k1][T[2]]);
+      }
+      v_off[p + 1] = v_off[p] + s;
+    }
+  }
+  return GWSIG_OK;
+}
+
+void Plan::g_source(int k2, long long& off, long long& tstride) const {
+  if (mode == GWSIG_IBZ_BLOCK) {
+    tstride = sumsq(ao_off[k2]);
+    if (general_gauge) {      // unfolded packed buffer over the whole mesh, mesh order
+      off = 0;
+      for (int k = 0; k < k2; ++k) off += sumsq(ao_off[k]) * ntau;
+    } else off = g_in_off[ir_index[ir_of[k2]]];          // S5 gauge: data of the representative
+  } else {
+    tstride = (long long)nao * nao;
+    off = (long long)k2 * ntau * tstride;               // dG itself (FULL_BZ) or the unfolded buffer (IBZ)
+  }
+}
+
+void Plan::w_source(int q, int q_first, long long& off, long long& tstride) const {
+  if (mode == GWSIG_IBZ_BLOCK) {
+    tstride = sumsq(aux_off[q]);
+    if (general_gauge) {
+      off = 0;
+      for (int k = q_first; k < q; ++k) off += sumsq(aux_off[k]) * ntau;
+    } else off = w_in_off[ir_index[ir_of[q]]];
+  } else {
+    tstride = (long long)naux * naux;
+    off = (long long)(mode == GWSIG_FULL_BZ ? q : q - q_first) * ntau * tstride;
+  }
+}
+
+static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo; d.div = GWSIG_NODIV; d.pad_ = 0; return d; }
+static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
+
+int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out) const {
+  out.prob.clear(); out.seg.clear(); out.ntiles = 0; out.shape_class = 0;
+  if (p0 < 0 || np < 1 || p0 + np > npairs || nt < 1 || nt > ntau || stage < 1 || stage > 3) return GWSIG_ERR_ARG;
+  if (v_off.empty()) return GWSIG_ERR_ARG;
+
+  // chunk-local X / Y offsets: [pair][tau in chunk][xsize(pair)]
+  std::vector<long long> xoff(np + 1, 0);
+  for (long long l = 0; l < np; ++l) xoff[l + 1] = xoff[l] + xsize(p0 + l) * nt;
+
+  struct TripleLay { int p, al, io, np_, na, ni; long long c0, poff, Np; };
+  auto pair_layout = [&](long long p, std::vector<TripleLay>& T, std::vector<long long>& Np, std::vector<long long>& poff, int& k1,
+                         int& k2, int& q, int& i1) {
+    pair(p, k1, k2, q, i1);
+    const std::vector<int>&oq = aux_off[q], &o2 = ao_off[k2], &o1 = ao_off[k1];
+    int nb = (int)oq.size() - 1;
+    Np.assign(nb, 0); poff.assign(nb + 1, 0);
+    int ntr = pair_ntriples(p);
+    T.resize(ntr);
+    for (int t = 0; t < ntr; ++t) {
+      int bp, ba, bi;
+      pair_triple(p, t, bp, ba, bi);
+      TripleLay& L = T[t];
+      L.p = bp; L.al = ba; L.io = bi;
+      L.np_ = oq[bp + 1] - oq[bp]; L.na = o2[ba + 1] - o2[ba]; L.ni = o1[bi + 1] - o1[bi];
+      L.c0 = Np[bp];
+      Np[bp] += (long long)L.na * L.ni;
+    }
+    for (int b = 0; b < nb; ++b) poff[b + 1] = poff[b] + (long long)(oq[b + 1] - oq[b]) * Np[b];
+    for (auto& L : T) { L.poff = poff[L.p]; L.Np = Np[L.p]; }
+  };
+  auto blk_off = [](const std::vector<int>& off, int b) {     // offset of diagonal block b in the packed layout
+    long long s = 0;
+    for (int c = 0; c < b; ++c) s += (long long)(off[c + 1] - off[c]) * (off[c + 1] - off[c]);
+    return s;
+  };
+
+  std::vector<TripleLay> T;
+  std::vector<long long> Np, poff;
+  std::vector<long long> cost;       // per problem: total K (tiles of one launch share the tile area)
+
+  if (stage == 1 || stage == 2) {
+    for (long long l = 0; l < np; ++l) {
+      const long long p = p0 + l;
+      int k1, k2, q, i1;
+      pair_layout(p, T, Np, poff, k1, k2, q, i1);
+      const long long vrel = v_off[p] - v_off[p0];
+      const long long xs = xsize(p);
+      if (stage == 1) {
+        long long goff, gts;
+        g_source(k2, goff, gts);
+        for (const auto& L : T) {
+          gwsig_seg S; std::memset(&S, 0, sizeof(S));
+          gwsig_problem P; std::memset(&P, 0, sizeof(P));
+          // X[P,i,b](tau) = sum_a conj(V2[P,a,i]) G[a,b](tau)          (Algorithm 4 line 5)
+          S.a_off = vrel + L.poff + L.c0;
+          S.am = lvl2(L.ni, L.Np, 1);                     // m = (P, i)
+          S.ak = lvl1(L.ni);                              // k = a
+          S.b_off = goff + blk_off(ao_off[k2], L.al);
+          S.bk = lvl1(L.na);
+          S.bn = lvl2(L.na, gts, 1);                      // n = (tau, b)
+          S.K = L.na;
+          P.M = L.np_ * L.ni; P.N = nt * L.na;
+          P.c_off = xoff[l] + L.poff + L.c0;
+          P.cm = lvl2(L.ni, L.Np, L.na);
+          P.cn = lvl2(L.na, xs, 1);
+          P.b_tstride = gts;
+          P.nbatch = 1;
+          P.flags = GWSIG_FLAG_CONJ_A;
+          P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+          out.seg.push_back(S); out.prob.push_back(P); cost.push_back(S.K);
+        }
+      } else {
+        long long woff, wts;
+        w_source(q, q_first, woff, wts);
+        const std::vector<int>& oq = aux_off[q];
+        for (int b = 0; b + 1 < (int)oq.size(); ++b) {
+          if (Np[b] == 0) continue;
+          const int npb = oq[b + 1] - oq[b];
+          gwsig_seg S; std::memset(&S, 0, sizeof(S));
+          gwsig_problem P; std::memset(&P, 0, sizeof(P));
+          // Y[P',n](tau) = sum_P W[P,P'](tau) X[P,n](tau)                (Algorithm 4 line 7)
+          S.a_off = woff + blk_off(oq, b);
+          S.am = lvl1(1); S.ak = lvl1(npb);
+          S.b_off = xoff[l] + poff[b];
+          S.bk = lvl1(Np[b]); S.bn = lvl1(1);
+          S.K = npb;
+          P.M = npb; P.N = (int)Np[b];
+          P.c_off = xoff[l] + poff[b];
+          P.cm = lvl1(Np[b]); P.cn = lvl1(1);
+          P.a_bstride = wts; P.a_tstride = wts;
+          P.b_bstride = xs; P.c_bstride = xs;
+          P.nbatch = nt;
+          P.flags = 0;
+          P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+          out.seg.push_back(S); out.prob.push_back(P); cost.push_back(S.K);
+        }
+      }
+    }
+  } else {
+    // stage 3: Sigma_iota[i,j](tau) += sum over the pairs of this range with the same k1 and their triples
+    //          with output block iota of  sum_{P',b} Y[P',i,b] V2[P',b,j]      (Algorithm 4 line 8, PAPER.md:347;
+    //          only diagonal (iota,iota) blocks: the others cancel in the q sum -- DESIGN.md A8)
+    int maxN = 0;
+    for (int i1 = 0; i1 < nk1; ++i1) {
+      const int k1 = out_list[i1];
+      const std::vector<int>& o1 = ao_off[k1];
+      const int nb1 = (int)o1.size() - 1;
+      std::vector<std::vector<gwsig_seg>> segs(nb1);
+      long long lfirst = ((long long)i1 - (p0 % nk1) + nk1) % nk1;
+      for (long long l = lfirst; l < np; l += nk1) {
+        const long long p = p0 + l;
+        int k1_, k2, q, i1_;
+        pair_layout(p, T, Np, poff, k1_, k2, q, i1_);
+        const long long vrel = v_off[p] - v_off[p0];
+        const long long xs = xsize(p);
+        for (const auto& L : T) {
+          gwsig_seg S; std::memset(&S, 0, sizeof(S));
+          S.a_off = xoff[l] + L.poff + L.c0;               // Y, same layout as X
+          S.am = lvl2(L.ni, xs, L.na);                     // m = (tau, i)
+          S.ak = lvl2(L.na, L.Np, 1);                      // k = (P', b)
+          S.b_off = vrel + L.poff + L.c0;
+          S.bk = lvl2(L.na, L.Np, L.ni);
+          S.bn = lvl1(1);
+          S.K = L.np_ * L.na;
+          segs[L.io].push_back(S);
+        }
+      }
+      long long sts = mode == GWSIG_IBZ_BLOCK ? sumsq(o1) : (long long)nao * nao;
+      for (int b = 0; b < nb1; ++b) {
+        if (segs[b].empty()) continue;
+        const int ni = o1[b + 1] - o1[b];
+        gwsig_problem P; std::memset(&P, 0, sizeof(P));
+        P.M = nt * ni; P.N = ni;
+        P.c_off = sig_off[i1] + blk_off(o1, b);
+        P.cm = lvl2(ni, sts, ni); P.cn = lvl1(1);
+        P.c_tstride = sts;
+        P.nbatch = 1;
+        P.flags = GWSIG_FLAG_ACCUM | GWSIG_FLAG_A_KMAJOR;
+        P.seg_begin = (int)out.seg.size(); P.seg_count = (int)segs[b].size();
+        long long kt = 0;
+        for (auto& S : segs[b]) { out.seg.push_back(S); kt += S.K; }
+        out.prob.push_back(P); cost.push_back(kt);
+        maxN = std::max(maxN, ni);
+      }
+    }
+    out.shape_class = maxN <= 32 ? 1 : 0;
+  }
+
+  // heaviest problems first (dynamic scheduler takes tiles in order), then the tile prefix
+  std::vector<int> order(out.prob.size());
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost[x] > cost[y]; });
+  std::vector<gwsig_problem> sorted(out.prob.size());
+  const ZgTile ts = zg_tile_shape(out.shape_class);
+  long long tb = 0;
+  for (size_t i = 0; i < order.size(); ++i) {
+    gwsig_problem P = out.prob[order[i]];
+    P.tiles_m = (P.M + ts.bm - 1) / ts.bm;
+    P.tiles_n = (P.N + ts.bn - 1) / ts.bn;
+    P.tile_begin = tb;
+    tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
+    sorted[i] = P;
+  }
+  out.prob.swap(sorted);
+  out.ntiles = tb;
+  return GWSIG_OK;
+}
+
+void Plan::flop_counts(double& full_equiv, double& executed) const {
+  const double A = (double)naux * nao * nao * nao, B = (double)naux * naux * nao * nao;
+  full_equiv = (double)nk * nk * ntau * 8.0 * (2.0 * A + B);
+  if (mode != GWSIG_IBZ_BLOCK) { executed = (double)npairs * ntau * 8.0 * (2.0 * A + B); return; }
+  executed = 0;
+  if (!have_triples) return;
+  double macs = 0;
+  for (long long p = 0; p < npairs; ++p) {
+    int k1, k2, q, i1;
+    pair(p, k1, k2, q, i1);
+    const std::vector<int>&oq = aux_off[q], &o2 = ao_off[k2], &o1 = ao_off[k1];
+    std::vector<double> Np(oq.size() - 1, 0.0);
+    for (long long t = triple_ptr[p]; t < triple_ptr[p + 1]; ++t) {
+      const int32_t* T = &triples[3 * t];
+      double np_ = oq[T[0] + 1] - oq[T[0]], na = o2[T[1] + 1] - o2[T[1]], ni = o1[T[2] + 1] - o1[T[2]];
+      macs += np_ * ni * na * na + np_ * na * ni * ni;      // stage 1 + stage 3
+      Np[T[0]] += na * ni;
+    }
+    for (size_t b = 0; b < Np.size(); ++b) { double npb = oq[b + 1] - oq[b]; macs += npb * npb * Np[b]; }   // stage 2
+  }
+  executed = 8.0 * ntau * macs;
+}
+
+}  // namespace gwsig

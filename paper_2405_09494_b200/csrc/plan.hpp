@@ -1,0 +1,108 @@
+// Host plan of the GW self-energy evaluation (step a0 of DESIGN.md): k maps, stars, pair list,
+// packed layouts, and the lowering of Algorithm 4 to grouped-GEMM descriptors.
+// Pure host C++ (no CUDA calls) so that it can be exercised without a device.
+#pragma once
+#include <complex>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "gwsig.h"
+#include "gwsig_plan.h"
+
+namespace gwsig {
+
+typedef std::complex<double> cplx;
+
+struct StagePlan {
+  std::vector<gwsig_problem> prob;
+  std::vector<gwsig_seg> seg;
+  long long ntiles = 0;
+  int shape_class = 0;
+};
+
+struct Plan {
+  // ---- lattice / sizes -------------------------------------------------------------------
+  double a[9] = {0};
+  int N[3] = {0, 0, 0};
+  int nk = 0, nao = 0, naux = 0, ntau = 0, natom = 0;
+  double beta = 0;
+  std::vector<double> pos;
+  std::vector<int> ao_atom, aux_atom;
+  bool have_lattice = false, have_atoms = false, have_sym = false, have_blocks = false, have_triples = false;
+
+  // ---- symmetry ---------------------------------------------------------------------------
+  int nops = 0, mode = GWSIG_FULL_BZ;
+  std::vector<int> rot;        // [nops][9]
+  std::vector<double> trans;   // [nops][3]
+  std::vector<double> D_ao, D_aux;
+  std::vector<int> shift;      // [nops][natom][3]
+  std::vector<int> rotk;       // [nops][nk]   k~ = k W^-1
+  std::vector<int> ir_list, ir_of, op_of, ir_index;   // ir_index[k] = position in ir_list or -1
+  std::vector<int> out_list;   // k1 values Sigma is produced for (wedge or all k)
+  int nk1 = 0;
+  long long npairs = 0;
+
+  // ---- blocks (IBZ_BLOCK) -------------------------------------------------------------------
+  std::vector<std::vector<int>> ao_off, aux_off;     // per k: nblk+1 offsets (trivial {0,n} in dense modes)
+  std::vector<cplx> U_ao, U_aux;                     // optional general gauge
+  bool general_gauge = false;
+  std::vector<long long> triple_ptr;                 // [npairs+1]
+  std::vector<int32_t> triples;                      // [3*nt]
+
+  // ---- packed layouts (complex elements) --------------------------------------------------------
+  std::vector<long long> g_in_off, w_in_off;   // per wedge/mesh point of the INPUT G / W buffers
+  std::vector<long long> sig_off;              // per out_list entry
+  std::vector<long long> v_off;                // [npairs+1]
+  long long g_elems = 0, w_elems = 0, sig_elems = 0;
+
+  std::string err;
+
+  // mesh arithmetic
+  int kindex(int n0, int n1, int n2) const;
+  int ksub(int k, int q) const;
+  void kcoords(int k, int n[3]) const;
+
+  int set_lattice(const double a_[9], const int mesh[3], int nao_, int naux_, int ntau_, double beta_);
+  int set_atoms(int natom_, const double* pos_, const int* ao_atom_, const int* aux_atom_);
+  int set_symmetry(int nops_, const int* rot_, const double* trans_, const double* D_ao_, const double* D_aux_,
+                   const int* shift_, int mode_);
+  int set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nblk_aux, const int* aux_block_off,
+                 const double* U_ao_, const double* U_aux_);
+  int set_triples(int64_t npairs_, const int64_t* triple_ptr_, const int32_t* triples_);
+  int finalize_layouts();
+
+  // pair decomposition (q-major)
+  void pair(long long p, int& k1, int& k2, int& q, int& i1) const {
+    q = (int)(p / nk1);
+    i1 = (int)(p % nk1);
+    k1 = out_list[i1];
+    k2 = ksub(k1, q);
+  }
+  // triples of a pair: explicit in block mode, the single dense triple (0,0,0) otherwise
+  int pair_ntriples(long long p) const { return mode == GWSIG_IBZ_BLOCK ? (int)(triple_ptr[p + 1] - triple_ptr[p]) : 1; }
+  void pair_triple(long long p, int t, int& bp, int& ba, int& bi) const {
+    if (mode == GWSIG_IBZ_BLOCK) {
+      const int32_t* T = &triples[3 * (triple_ptr[p] + t)];
+      bp = T[0]; ba = T[1]; bi = T[2];
+    } else { bp = ba = bi = 0; }
+  }
+  long long xsize(long long p) const { return v_off[p + 1] - v_off[p]; }   // X, Y and V2 share the shape
+
+  // where the contraction reads G(k2) / W(q) from and with what tau stride.  q_first: first q held by
+  // the W ring (IBZ dense mode).
+  void g_source(int k2, long long& off, long long& tstride) const;
+  void w_source(int q, int q_first, long long& off, long long& tstride) const;
+
+  // lowering to descriptors; stage 1..3 as in gwsig_plan_get()
+  int build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out) const;
+  void flop_counts(double& full_equiv, double& executed) const;
+};
+
+static inline long long sumsq(const std::vector<int>& off) {
+  long long s = 0;
+  for (size_t b = 0; b + 1 < off.size(); ++b) s += (long long)(off[b + 1] - off[b]) * (off[b + 1] - off[b]);
+  return s;
+}
+
+}  // namespace gwsig

@@ -1,0 +1,129 @@
+"""Test-side helpers: fold Sigma back to the orbital basis on the full zone (Eq. 26, 22) and a
+numpy interpreter of the library's grouped-GEMM descriptors (checks the HOST plan without a GPU).
+Nothing here is used by the product path."""
+import numpy as np
+
+from gwsig_synth.group import rep_at_k
+from paper_2405_09494_b200.binding import (FLAG_ACCUM, FLAG_CONJ_A, FLAG_CONJ_B, FULL_BZ, IBZ, IBZ_BLOCK, NODIV)
+
+
+def oracle_sigma(inp, ks, taus=None):
+    from oracle.sigma_oracle import sigma_ref
+    taus = np.arange(inp.ntau) if taus is None else np.asarray(taus)
+    cache_g, cache_w = {}, {}
+
+    def G_of(k):
+        if k not in cache_g:
+            cache_g[k] = (inp.G_k(k) if hasattr(inp, "G_k") else inp.G_full()[k])[taus]
+        return cache_g[k]
+
+    def W_of(q):
+        if q not in cache_w:
+            cache_w[q] = inp.W_full([q])[0][taus]
+        return cache_w[q]
+
+    return sigma_ref(inp.nk, inp.kmesh.sub, G_of, W_of, inp.V_pair, ks)
+
+
+def fold_to_orbital(cfg, inp, sigma_list):
+    """list over cfg.out_list of [nt, nao, nao] (basis of the mode) -> dict k -> [nt, nao, nao] in the
+    orbital basis for EVERY mesh point: Sigma_orb(k_I) = U Sigma_blk U^dagger (Eq. 26), then
+    Sigma(k') = O Sigma(k_I) O^dagger (Eq. 22)."""
+    out = {}
+    for i, k in enumerate(cfg.out_list):
+        S = sigma_list[i]
+        if cfg.mode == IBZ_BLOCK:
+            U = cfg.ao.U[k]
+            S = U @ S @ U.conj().T
+        out[int(k)] = S
+    if cfg.mode == FULL_BZ:
+        return out
+    cr = inp.cr
+    for k in range(cfg.nk):
+        if k in out:
+            continue
+        g = int(cfg.op_of[k])
+        O = rep_at_k(cr.P_ao[g], cr.ao_atom, cr.sg.shift[g], cr.kmesh.frac[k])
+        out[k] = O @ out[int(cfg.ir_of[k])] @ O.conj().T
+    return out
+
+
+def rel_err(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def _idx(d, n):
+    i = np.arange(n, dtype=np.int64)
+    if d["div"] == NODIV:
+        return i * d["lo"]
+    return (i // d["div"]) * d["hi"] + (i % d["div"]) * d["lo"]
+
+
+def run_stage_numpy(prob, seg, A, B, C, t0):
+    """execute one stage's descriptors exactly as documented in include/gwsig_plan.h."""
+    for P in prob:
+        cm, cn = _idx(P["cm"], P["M"]), _idx(P["cn"], P["N"])
+        for bt in range(P["nbatch"]):
+            acc = np.zeros((P["M"], P["N"]), complex)
+            for s in range(P["seg_begin"], P["seg_begin"] + P["seg_count"]):
+                S = seg[s]
+                a0 = S["a_off"] + bt * P["a_bstride"] + t0 * P["a_tstride"]
+                b0 = S["b_off"] + bt * P["b_bstride"] + t0 * P["b_tstride"]
+                Am = A[a0 + _idx(S["am"], P["M"])[:, None] + _idx(S["ak"], S["K"])[None, :]]
+                Bm = B[b0 + _idx(S["bk"], S["K"])[:, None] + _idx(S["bn"], P["N"])[None, :]]
+                if P["flags"] & FLAG_CONJ_A:
+                    Am = Am.conj()
+                if P["flags"] & FLAG_CONJ_B:
+                    Bm = Bm.conj()
+                acc += Am @ Bm
+            ci = P["c_off"] + bt * P["c_bstride"] + t0 * P["c_tstride"] + cm[:, None] + cn[None, :]
+            if P["flags"] & FLAG_ACCUM:
+                C[ci] += acc
+            else:
+                C[ci] = acc
+
+
+def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
+    """emulate gwsig_sigma_eval's orchestration with the descriptors of gwsig_plan_get()."""
+    lib = cfg.lib
+    ntau, nao, naux, nk = cfg.ntau, cfg.nao, cfg.naux, cfg.nk
+    nt = ntau if nt is None else nt
+    push_pairs = cfg.npairs if push_pairs is None else push_pairs
+    sig_elems = lib.buffer_sizes()[2]
+    acc = np.zeros(sig_elems, complex)
+    # G / W sources
+    if cfg.mode == IBZ:
+        cr = inp.cr
+        Gi = G_flat.reshape(len(cfg.ir_list), ntau, nao, nao)
+        Wi = W_flat.reshape(len(cfg.ir_list), ntau, naux, naux)
+        ir_index = {int(k): i for i, k in enumerate(cfg.ir_list)}
+
+        def unfold(X, P, atom, k):
+            g = int(cfg.op_of[k])
+            O = rep_at_k(P[g], atom, cr.sg.shift[g], cr.kmesh.frac[k])
+            return O @ X[ir_index[int(cfg.ir_of[k])]] @ O.conj().T
+        Gsrc = np.stack([unfold(Gi, cr.P_ao, cr.ao_atom, k) for k in range(nk)]).ravel()
+    else:
+        Gsrc = G_flat
+    voff = [lib.pair_info(p)[3] for p in range(cfg.npairs)] + [V_flat.size]
+    p0 = 0
+    while p0 < cfg.npairs:
+        npp = min(push_pairs, cfg.npairs - p0)
+        q_first, q_last = p0 // cfg.nk1, (p0 + npp - 1) // cfg.nk1
+        if cfg.mode == IBZ:
+            Wsrc = np.stack([unfold(Wi, cr.P_aux, cr.aux_atom, q) for q in range(q_first, q_last + 1)]).ravel()
+        else:
+            Wsrc = W_flat
+        Vsub = V_flat[voff[p0]:voff[p0 + npp]]
+        for t0 in range(0, ntau, nt):
+            ntc = min(nt, ntau - t0)
+            X = np.zeros(Vsub.size * ntc, complex)
+            Y = np.zeros(Vsub.size * ntc, complex)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 1)
+            run_stage_numpy(pr, sg, Vsub, Gsrc, X, t0)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 2)
+            run_stage_numpy(pr, sg, Wsrc, X, Y, t0)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 3)
+            run_stage_numpy(pr, sg, Y, Vsub, acc, t0)
+        p0 += npp
+    return -acc / nk

@@ -1,0 +1,124 @@
+"""Host logic of the C-ABI library, no GPU: the library loads and exports every declared symbol, the
+plan (stars, pair list, layouts) is right, error conventions hold, and the grouped-GEMM descriptors --
+executed by a numpy interpreter -- reproduce the oracle in all three modes."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from gwsig_synth import make_inputs
+from paper_2405_09494_b200 import build as gw_build
+
+gw_build.build()
+from paper_2405_09494_b200 import binding as B                                   # noqa: E402
+from paper_2405_09494_b200.pack import Configured, configure_from_crystal        # noqa: E402
+from tests.helpers import fold_to_orbital, oracle_sigma, rel_err, run_plan_numpy  # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "gwsig.h")).read()
+    declared = set(re.findall(r"\b(gwsig_[a-z0-9_]+)\s*\(", hdr))
+    declared -= {"gwsig_ctx", "gwsig_status", "gwsig_mode", "gwsig_engine"}
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for name in sorted(declared):
+        assert hasattr(lib, name), name
+    assert declared == set(B.EXPORTS)
+
+
+def test_struct_layouts_match_header():
+    assert (B.IDX2.itemsize, B.SEG.itemsize, B.PROBLEM.itemsize) == (24, 120, 144)
+
+
+def test_no_cpu_fallback_without_device():
+    lib = B.Gwsig(device=-1)
+    inp = make_inputs("cfg1", mesh=(2, 1, 1), nao=2, naux=2, ntau=2, nocc=1)
+    cfg = Configured(lib, B.FULL_BZ, np.eye(3), (2, 1, 1), 2, 2, 2, 1.0, None, None, None)
+    z = np.zeros(64, complex)
+    with pytest.raises(B.GwsigError) as e:
+        lib.sigma_eval(z, z, z, z)
+    assert e.value.code == -4 and "no CPU fallback" in str(e.value)
+
+
+def test_stars_and_pairs_match_setup():
+    inp = make_inputs("toy_diamond4")
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ)
+    st = cfg.setup
+    assert np.array_equal(cfg.ir_list, st.ir_list) and np.array_equal(cfg.ir_of, st.ir_of) and np.array_equal(cfg.op_of, st.op_of)
+    assert len(cfg.ir_list) == 8                       # Table 2, Si 4x4x4
+    assert cfg.npairs == 64 * 8
+    for p in (0, 7, 8, 100, 511):
+        k1, k2, q, off, ne = lib.pair_info(p)
+        assert q == p // 8 and k1 == cfg.ir_list[p % 8] and k2 == st.sub(k1, q)
+        assert off == p * inp.naux * inp.nao ** 2 and ne == inp.naux * inp.nao ** 2
+    full, ex = lib.flop_counts()
+    unit = inp.ntau * 8 * (2 * inp.naux * inp.nao ** 3 + inp.naux ** 2 * inp.nao ** 2)
+    assert full == 64 * 64 * unit and ex == 64 * 8 * unit
+
+
+def test_error_conventions():
+    inp = make_inputs("toy_sc")
+    cr, sg = inp.cr, inp.cr.sg
+    lib = B.Gwsig(device=-1)
+    with pytest.raises(B.GwsigError) as e:
+        lib.set_lattice(cr.a, (2, 2, 0), cr.nao, cr.naux, 2, 1.0)
+    assert e.value.code == -1
+    lib.set_lattice(cr.a, (2, 3, 2), cr.nao, cr.naux, 2, 1.0)
+    lib.set_atoms(cr.pos, cr.ao_atom, cr.aux_atom)
+    with pytest.raises(B.GwsigError) as e:              # cubic rotations do not map a 2x3x2 mesh onto itself
+        lib.set_symmetry(sg.W, sg.w, cr.P_ao, cr.P_aux, sg.shift, B.IBZ)
+    assert e.value.code == -2
+    lib.set_lattice(cr.a, cr.mesh, cr.nao, cr.naux, 2, 1.0)
+    lib.set_atoms(cr.pos, cr.ao_atom, cr.aux_atom)
+    bad = cr.P_ao.copy(); bad[3, 0, 0] += 0.1
+    with pytest.raises(B.GwsigError) as e:              # non-orthogonal representation matrix
+        lib.set_symmetry(sg.W, sg.w, bad, cr.P_aux, sg.shift, B.IBZ)
+    assert e.value.code == -2
+    lib.set_symmetry(sg.W, sg.w, cr.P_ao, cr.P_aux, sg.shift, B.IBZ_BLOCK)
+    nk = lib.nk
+    with pytest.raises(B.GwsigError) as e:              # blocks that do not tile [0, nao)
+        lib.set_blocks([np.array([0, cr.nao - 1])] * nk, [np.array([0, cr.naux])] * nk)
+    assert e.value.code == -3
+    with pytest.raises(B.GwsigError) as e:              # a star member whose blocks differ from its representative's
+        offs = [np.array([0, cr.nao])] * nk
+        offs[1] = np.array([0, 1, cr.nao])
+        lib.set_blocks(offs, [np.array([0, cr.naux])] * nk)
+    assert e.value.code == -3
+    lib.set_blocks([np.array([0, cr.nao])] * nk, [np.array([0, cr.naux])] * nk)
+    npairs, _ = lib.pair_count()
+    with pytest.raises(B.GwsigError) as e:              # triple with a block index out of range
+        lib.set_triples(np.arange(npairs + 1), np.tile([0, 1, 0], (npairs, 1)))
+    assert e.value.code == -3
+
+
+@pytest.mark.parametrize("name,mode,push,nt", [
+    ("cfg1s", B.FULL_BZ, None, None), ("cfg1s", B.FULL_BZ, 8, 1),
+    ("toy_diamond", B.IBZ, None, None), ("toy_diamond", B.IBZ, 6, 2),
+    ("toy_diamond", B.IBZ_BLOCK, None, None), ("toy_diamond", B.IBZ_BLOCK, 3, 2),
+    ("toy_wurtzite", B.IBZ_BLOCK, None, None), ("toy_rocksalt", B.IBZ_BLOCK, 9, None),
+])
+def test_descriptors_reproduce_oracle(name, mode, push, nt):
+    lib = B.Gwsig(device=-1)
+    if name == "cfg1s":
+        inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=5, ntau=3, beta=4.0, nocc=1, seed=2)
+        cfg = Configured(lib, mode, np.eye(3), (2, 2, 1), 3, 5, 3, 4.0, None, None, None)
+        Gf, Wf = inp.G_full(), inp.W_full()
+        G, W = cfg.pack_GW(lambda k: Gf[k], lambda q: Wf[q])
+    else:
+        inp = make_inputs(name)
+        cfg = configure_from_crystal(lib, inp.cr, mode)
+        G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    V = cfg.pack_V(inp.V2_rows)
+    sig = run_plan_numpy(cfg, inp, G, W, V, push_pairs=push, nt=nt)
+    got = fold_to_orbital(cfg, inp, cfg.unpack_sigma(sig))
+    ref = oracle_sigma(inp, range(inp.nk))
+    for k in range(inp.nk):
+        for t in range(inp.ntau):
+            assert rel_err(got[k][t], ref[k, t]) < 1e-12, (k, t)
+    if mode == B.IBZ_BLOCK:
+        full, ex = lib.flop_counts()
+        assert 0 < ex < full * len(cfg.ir_list) / inp.nk
