@@ -51,6 +51,17 @@ typedef enum {
   GWSIG_ENGINE_REFERENCE = 1 /* one-thread-per-element DFMA kernels on the same plan (debug)      */
 } gwsig_engine;
 
+/* kernel kinds for gwsig_kernel_times (steps a1..a6 of DESIGN.md) */
+enum {
+  GWSIG_KIND_UNFOLD_G = 0,
+  GWSIG_KIND_UNFOLD_W = 1,
+  GWSIG_KIND_STAGE1 = 2, /* X = V G          */
+  GWSIG_KIND_STAGE2 = 3, /* Y = W X          */
+  GWSIG_KIND_STAGE3 = 4, /* Sigma += Y V     */
+  GWSIG_KIND_EPILOGUE = 5,
+  GWSIG_NKINDS = 6
+};
+
 /* ---- life cycle ------------------------------------------------------------------------ */
 /* device >= 0: CUDA device ordinal used by sigma_*; device < 0: host-only context (plan calls). */
 int gwsig_create(gwsig_ctx** out, int device);
@@ -132,14 +143,19 @@ int gwsig_sigma_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, const v
 
 /* ---- options and accounting ------------------------------------------------------------------ */
 /* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
- * default 4096), "tau_chunk" (0 = from the budget)                                                */
+ * default 8192), "tau_chunk" (0 = from the budget), "timing" (0/1: record a CUDA event pair around
+ * every kernel launch on the launching stream, read back with gwsig_kernel_times)                  */
 int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value);
 /* real flops (8 per complex multiply-add) of one evaluation: the full-BZ dense equivalent
  * Nk^2 ntau 8(2A+B) and what the current mode's plan actually asks for.
  * In IBZ_BLOCK mode `executed` needs set_triples first.                                            */
 int gwsig_flop_counts(gwsig_ctx* ctx, double* full_bz_equiv, double* executed);
-/* number of kernel launches and DMMA-engine device time bookkeeping of the last evaluation         */
+/* number of kernel launches of the last evaluation                                                 */
 int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
+/* device time (ms, CUDA events on the launching stream) and launch count per kernel kind of the last
+ * evaluation; ms[GWSIG_NKINDS], launches[GWSIG_NKINDS] (host).  Needs option "timing" = 1; blocks
+ * until the last recorded event has completed.                                                     */
+int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
  * stage: 1 = X = V G, 2 = Y = W X, 3 = Sigma += Y V, 4 = unfold step 1, 5 = unfold step 2.

@@ -34,7 +34,7 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_set_symmetry", "gwsig_set_blocks", "gwsig_set_triples", "gwsig_get_ibz", "gwsig_pair_count",
            "gwsig_pair_info", "gwsig_buffer_sizes", "gwsig_sigma_begin", "gwsig_sigma_push_pairs", "gwsig_sigma_end",
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
-           "gwsig_plan_get", "gwsig_probe_fp64"]
+           "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -48,7 +48,7 @@ _sig = {
     "gwsig_sigma_eval": [_vp, _vp, _vp, _vp, _vp, _vp], "gwsig_set_option": [_vp, C.c_char_p, _i64],
     "gwsig_flop_counts": [_vp, _vp, _vp], "gwsig_last_launch_count": [_vp, _vp],
     "gwsig_plan_counts": [_vp, _i64, _i64, _i, _i, _vp, _vp, _vp], "gwsig_plan_get": [_vp, _i64, _i64, _i, _i, _vp, _vp],
-    "gwsig_probe_fp64": [_vp, _i, _i, _i, _i64, _vp, _vp],
+    "gwsig_probe_fp64": [_vp, _i, _i, _i, _i64, _vp, _vp], "gwsig_kernel_times": [_vp, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -172,6 +172,14 @@ class Gwsig:
         n = C.c_int64()
         self._ck(_lib.gwsig_last_launch_count(self._h, C.addressof(n)))
         return n.value
+
+    KINDS = ("unfold_G", "unfold_W", "stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV", "epilogue")
+
+    def kernel_times(self):
+        ms = np.zeros(6, np.float64)
+        n = np.zeros(6, np.int64)
+        self._ck(_lib.gwsig_kernel_times(self._h, ms.ctypes.data, n.ctypes.data))
+        return {k: (float(m), int(c)) for k, m, c in zip(self.KINDS, ms, n)}
 
     def set_option(self, key, value):
         self._ck(_lib.gwsig_set_option(self._h, key.encode(), int(value)))

@@ -80,6 +80,12 @@ struct gwsig_ctx {
   std::map<std::tuple<long long, long long, int, int>, std::unique_ptr<DevPlan>> plan_cache;
   int counter_slot = 0;
   static constexpr int kCounterSlots = 8192;
+  // optional per-kernel device timing (option "timing"): event pairs on the launching stream
+  int timing = 0;
+  std::vector<cudaEvent_t> ev_pool;
+  std::vector<std::pair<int, int>> ev_used;     // (kind, pool index of the start event; stop = +1)
+  double kind_ms[GWSIG_NKINDS] = {0};
+  long long kind_launches[GWSIG_NKINDS] = {0};
 };
 
 namespace {
@@ -229,7 +235,26 @@ int get_dev_plan(gwsig_ctx* ctx, long long p0, long long np, int nt, int q_first
   return GWSIG_OK;
 }
 
-int run_stage(gwsig_ctx* ctx, const DevStage& d, const double2* A, const double2* B, double2* C, int t0) {
+int tic(gwsig_ctx* ctx, int kind) {
+  if (!ctx->timing) return GWSIG_OK;
+  size_t need = 2 * (ctx->ev_used.size() + 1);
+  while (ctx->ev_pool.size() < need) {
+    cudaEvent_t e;
+    CU(cudaEventCreate(&e));
+    ctx->ev_pool.push_back(e);
+  }
+  int idx = (int)(2 * ctx->ev_used.size());
+  ctx->ev_used.push_back(std::make_pair(kind, idx));
+  CU(cudaEventRecord(ctx->ev_pool[idx], ctx->stream));
+  return GWSIG_OK;
+}
+int toc(gwsig_ctx* ctx) {
+  if (!ctx->timing) return GWSIG_OK;
+  CU(cudaEventRecord(ctx->ev_pool[ctx->ev_used.back().second + 1], ctx->stream));
+  return GWSIG_OK;
+}
+
+int run_stage(gwsig_ctx* ctx, int kind, const DevStage& d, const double2* A, const double2* B, double2* C, int t0) {
   if (d.ntiles <= 0) return GWSIG_OK;
   if (ctx->counter_slot >= gwsig_ctx::kCounterSlots) {
     CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
@@ -243,7 +268,10 @@ int run_stage(gwsig_ctx* ctx, const DevStage& d, const double2* A, const double2
   zp.total_tiles = d.ntiles;
   zp.t0 = t0;
   zp.counter = (unsigned long long*)ctx->counters.p + ctx->counter_slot++;
+  int rc = tic(ctx, kind);
+  if (rc) return rc;
   CU(zg_launch(ctx->engine, d.shape_class, zp, ctx->num_sms, ctx->stream));
+  if ((rc = toc(ctx))) return rc;
   ctx->launches++;
   return GWSIG_OK;
 }
@@ -381,6 +409,7 @@ int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
     ctx->engine = (int)value;
   } else if (k == "hermitize") ctx->hermitize = value != 0;
   else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
+  else if (k == "timing") ctx->timing = value != 0;
   else if (k == "tau_chunk") { if (value < 0) return fail(ctx, GWSIG_ERR_ARG, "set_option: tau_chunk < 0"); ctx->tau_chunk = (int)value; }
   else return fail(ctx, GWSIG_ERR_ARG, "set_option: unknown key " + k);
   return GWSIG_OK;
@@ -399,6 +428,22 @@ int gwsig_flop_counts(gwsig_ctx* ctx, double* full_bz_equiv, double* executed) {
 int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches) {
   if (!ctx || !launches) return GWSIG_ERR_ARG;
   *launches = ctx->launches;
+  return GWSIG_OK;
+}
+
+int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches) {
+  if (!ctx || !ms || !launches) return GWSIG_ERR_ARG;
+  if (!ctx->timing) return fail(ctx, GWSIG_ERR_ARG, "kernel_times: set option timing = 1 before sigma_begin");
+  for (int i = 0; i < GWSIG_NKINDS; ++i) { ms[i] = 0; launches[i] = 0; }
+  if (!ctx->ev_used.empty()) {
+    CU(cudaEventSynchronize(ctx->ev_pool[ctx->ev_used.back().second + 1]));
+    for (auto& u : ctx->ev_used) {
+      float t = 0;
+      CU(cudaEventElapsedTime(&t, ctx->ev_pool[u.second], ctx->ev_pool[u.second + 1]));
+      ms[u.first] += t;
+      launches[u.first] += 1;
+    }
+  }
   return GWSIG_OK;
 }
 
@@ -450,6 +495,7 @@ int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSig
   CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
   ctx->counter_slot = 0;
   ctx->launches = 0;
+  ctx->ev_used.clear();
   if (P.mode == GWSIG_IBZ) {
     // [a1] G(k') = O G(k_I) O^dagger for every mesh point (Eq. 22; Algorithm 2 step 2)
     CU(ctx->gbz.ensure((size_t)P.nk * P.ntau * P.nao * P.nao * sizeof(double2)));
@@ -460,7 +506,9 @@ int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSig
     up.ell_cols = (const int*)ctx->ell_cols_ao.p; up.ell_vals = (const double*)ctx->ell_vals_ao.p;
     up.ell_cnt = (const int*)ctx->ell_cnt_ao.p;
     up.n = P.nao; up.ntau = P.ntau; up.maxnz = ctx->maxnz_ao;
+    if ((rc = tic(ctx, GWSIG_KIND_UNFOLD_G))) return rc;
     CU(launch_unfold_sparse(up, P.nk, ctx->stream));
+    if ((rc = toc(ctx))) return rc;
     ctx->launches++;
   }
   ctx->next_pair = 0;
@@ -492,7 +540,10 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
     up.ell_cols = (const int*)ctx->ell_cols_aux.p; up.ell_vals = (const double*)ctx->ell_vals_aux.p;
     up.ell_cnt = (const int*)ctx->ell_cnt_aux.p;
     up.n = P.naux; up.ntau = P.ntau; up.maxnz = ctx->maxnz_aux;
+    int rc = tic(ctx, GWSIG_KIND_UNFOLD_W);
+    if (rc) return rc;
     CU(launch_unfold_sparse(up, nq, ctx->stream));
+    if ((rc = toc(ctx))) return rc;
     ctx->launches++;
     Wsrc = (const double2*)ctx->wring.p;
   }
@@ -524,9 +575,9 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       DevPlan* dp = nullptr;
       int rc = get_dev_plan(ctx, s0, ns, ntc, q_first, &dp);
       if (rc) return rc;
-      if ((rc = run_stage(ctx, dp->st[0], Vsub, Gsrc, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
-      if ((rc = run_stage(ctx, dp->st[1], Wsrc, (const double2*)ctx->xbuf.p, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
-      if ((rc = run_stage(ctx, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Vsub, Gsrc, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], Wsrc, (const double2*)ctx->xbuf.p, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
     }
     s0 = s1;
   }
@@ -547,7 +598,10 @@ int gwsig_sigma_end(gwsig_ctx* ctx) {
   ep.desc = (const EpiDesc*)ctx->epidesc.p;
   ep.scale = -1.0 / (double)P.nk;
   ep.hermitize = ctx->hermitize;
+  int rc = tic(ctx, GWSIG_KIND_EPILOGUE);
+  if (rc) return rc;
   CU(launch_epilogue(ep, ctx->n_epidesc, ctx->num_sms, ctx->stream));
+  if ((rc = toc(ctx))) return rc;
   ctx->launches++;
   ctx->in_eval = false;
   return GWSIG_OK;

@@ -411,6 +411,7 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
         pair_layout(p, T, Np, poff, k1_, k2, q, i1_);
         const long long vrel = v_off[p] - v_off[p0];
         const long long xs = xsize(p);
+        if (xs * nt >= (1LL << 31)) return GWSIG_ERR_ARG;   // the k-major loader keeps 32-bit row offsets
         for (const auto& L : T) {
           gwsig_seg S; std::memset(&S, 0, sizeof(S));
           S.a_off = xoff[l] + L.poff + L.c0;               // Y, same layout as X

@@ -1,15 +1,17 @@
 // Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a).
 //
 // Serves the three contraction stages of the GW self-energy (Algorithm 4 lines 5, 7, 8 of
-// arXiv 2405.09494) and the block-basis unfold (Eq. 28).
-// Descriptors: include/gwsig_plan.h.  Design notes: DESIGN.md section 5.
+// arXiv 2405.09494).  Descriptors: include/gwsig_plan.h.  Design: DESIGN.md section 5.
 //
-//  * persistent CTAs, dynamic tile scheduler (one atomic per tile, heaviest problems first)
-//  * operands staged global -> shared with 16-byte cp.async (one complex128 per copy, so every
-//    two-level ragged index is addressable and ragged edges are zero-filled), STAGES-deep ring
+//  * persistent CTAs, dynamic tile scheduler over a cost-sorted tile list (heaviest problems first)
+//  * warp-specialised: ONE PRODUCER WARP does all index arithmetic (two-level ragged addressing) and
+//    stages operands global -> shared with 16-byte cp.async (one complex128 per copy; ragged edges are
+//    zero-filled), signalling a STAGES-deep ring of mbarriers (cp.async.mbarrier.arrive.noinc);
+//    the CONSUMER WARPS only wait, load fragments and issue DMMA, then release the slot
 //  * shared tiles are k-major with leading dimension = 2 (mod 8) complex elements: the
 //    one-double2-per-lane fragment loads of mma.m8n8k4.f64 are bank-conflict free
-//  * complex product = 4 real DMMA per 8x8x4 tile: re += ar*br, re += (-ai)*bi, im += ar*bi, im += ai*br
+//  * complex product = 4 real DMMA per 8x8x4 tile: re += ar*br, im += ar*bi, re += (-ai)*bi, im += ai*br,
+//    issued in two passes over the warp tile so that dependent DMMAs are MI*NI*2 instructions apart
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -23,15 +25,29 @@ __device__ __forceinline__ long long idx2(const gwsig_idx2& d, int i) {
   return (long long)q * d.hi + (long long)(i - q * d.div) * d.lo;
 }
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src, bool valid) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+__device__ __forceinline__ void cp_async16(unsigned smem_dst, const void* gmem_src, bool valid) {
   int bytes = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem_src), "r"(bytes));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gmem_src), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared.b64 st, [%0];\n\t}\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cp_async(unsigned bar) {   // fires when this thread's prior cp.async land
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n\t"
+      "@p bra WAIT_DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "WAIT_DONE:\n\t}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
 }
 
 // D(8x8) += A(8x4) * B(4x8), FP64 tensor core.  SASS: DMMA.8x8x4
@@ -52,206 +68,301 @@ __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long til
     if (__ldg(&p.prob[mid].tile_begin) <= tile) lo = mid; else hi = mid - 1;
   }
   const gwsig_problem& P = p.prob[lo];
-  long long local = tile - P.tile_begin;
-  int per = P.tiles_m * P.tiles_n;
+  long long local = tile - __ldg(&P.tile_begin);
+  int tn_ = __ldg(&P.tiles_n);
+  int per = __ldg(&P.tiles_m) * tn_;
   TileInfo t;
   t.prob = lo;
   t.batch = (int)(local / per);
   int r = (int)(local - (long long)t.batch * per);
-  t.tm = r / P.tiles_n;
-  t.tn = r - t.tm * P.tiles_n;
+  t.tm = r / tn_;
+  t.tn = r - t.tm * tn_;
   return t;
 }
 
 // ------------------------------------------------------------------------------------------
-// tensor-core engine
+// tensor-core engine, warp-specialised
+//   consumer warps: WGM x WGN, each owning an (8 MI) x (8 NI) complex tile; producer: 1 warp
+//   The producer owns the tile scheduler (one atomicAdd per tile) and every descriptor read; it
+//   tells the consumers what a pipeline slot holds through a small header in shared memory.
 // ------------------------------------------------------------------------------------------
-template <int BM, int BN, int WARPS_M, int WARPS_N, int STAGES>
-__global__ void __launch_bounds__(WARPS_M* WARPS_N * 32) zgemm_grouped_dmma(ZgParams p) {
+struct SlotHdr {
+  int ctl;            // bit0: first slot of a tile, bit1: last slot of a tile, bit2: no more work
+  int nk4;            // k4-steps of this slot that hold data (1 or 2)
+  int trec;           // index of the tile record (valid when bit0)
+  int pad_;
+};
+struct __align__(16) TileRec {   // what the consumers need to know about a tile (written by the producer)
+  int m_rem, n_rem;   // M - m0, N - n0
+  int flags, pad_;
+  long long c_off;    // element offset of C(m = 0, n = 0) incl. batch / tau offsets
+  int m0, n0;
+  gwsig_idx2 cm, cn;
+};
+
+template <int MI, int NI, int WGM, int WGN, int STAGES, int MAXREG>
+__global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm_grouped_dmma(ZgParams p) {
   constexpr int BK = 8;
-  constexpr int NT = WARPS_M * WARPS_N * 32;
-  constexpr int WTM = BM / WARPS_M, WTN = BN / WARPS_N;
-  constexpr int MI = WTM / 8, NI = WTN / 8;
+  constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
+  constexpr int NCW = WGM * WGN;                     // consumer warps
   constexpr int LDA = BM + 2, LDB = BN + 2;          // = 2 (mod 8): conflict-free fragment loads
-  constexpr int A_PER = (BM * BK) / NT, B_PER = (BN * BK) / NT;
-  static_assert((BM * BK) % NT == 0 && (BN * BK) % NT == 0, "tile / thread mismatch");
-  static_assert(BM % 8 == 0 && BN % 8 == 0 && LDA % 8 == 2 && LDB % 8 == 2, "layout");
+  constexpr int RA = (BM + 31) / 32, RB = (BN + 31) / 32;
+  constexpr int RAK = BM / 4;                        // rows per lane in the k-major A mapping
+  static_assert(LDA % 8 == 2 && LDB % 8 == 2 && BM % 4 == 0, "layout");
 
   extern __shared__ double2 zg_smem[];
-  double2* As = zg_smem;                           // [STAGES][BK][LDA]
-  double2* Bs = zg_smem + STAGES * BK * LDA;       // [STAGES][BK][LDB]
-  __shared__ unsigned long long s_tile;
+  double2* As = zg_smem;                             // [STAGES][BK][LDA]
+  double2* Bs = zg_smem + STAGES * BK * LDA;         // [STAGES][BK][LDB]
+  __shared__ __align__(8) unsigned long long bars[2 * STAGES];
+  __shared__ SlotHdr hdr[STAGES];
+  __shared__ TileRec trec[STAGES + 1];        // the producer is at most STAGES tiles ahead of any consumer
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm0 = (warp / WARPS_N) * WTM, wn0 = (warp % WARPS_N) * WTN;
-  const int fr = lane >> 2, fk = lane & 3;         // fragment row / k index of this lane
-
-  while (true) {
-    __syncthreads();                                // previous tile fully consumed (smem, s_tile)
-    if (tid == 0) s_tile = atomicAdd(p.counter, 1ULL);
-    __syncthreads();
-    const long long tile = (long long)s_tile;
-    if (tile >= p.total_tiles) break;
-
-    const TileInfo ti = decode_tile(p, tile);
-    const gwsig_problem& P = p.prob[ti.prob];
-    const int M = P.M, N = P.N, flags = P.flags;
-    const int m0 = ti.tm * BM, n0 = ti.tn * BN;
-    const long long a_boff = (long long)ti.batch * P.a_bstride + (long long)p.t0 * P.a_tstride;
-    const long long b_boff = (long long)ti.batch * P.b_bstride + (long long)p.t0 * P.b_tstride;
-    const bool kmajor = (flags & GWSIG_FLAG_A_KMAJOR) != 0;
-    const bool conjA = (flags & GWSIG_FLAG_CONJ_A) != 0, conjB = (flags & GWSIG_FLAG_CONJ_B) != 0;
-
-    // this thread's slots in the A and B tiles
-    int a_ml[A_PER], a_kl[A_PER], b_nl[B_PER], b_kl[B_PER];
+  const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
+  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[STAGES]);
+  if (tid == 0) {
 #pragma unroll
-    for (int e = 0; e < A_PER; ++e) {
-      int lin = tid + e * NT;
-      if (kmajor) { a_kl[e] = lin % BK; a_ml[e] = lin / BK; }
-      else        { a_ml[e] = lin % BM; a_kl[e] = lin / BM; }
-    }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 33); mbar_init(empty0 + 8 * s, NCW); }
+  }
+  __syncthreads();
+
+  int stage = 0;
+  unsigned phase = 0;
+
+  if (warp == NCW) {
+    // ================================= PRODUCER =================================================
+    const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
+    int tslot = 0;
+    while (true) {
+      long long tile = 0;
+      if (lane == 0) tile = (long long)atomicAdd(p.counter, 1ULL);
+      tile = __shfl_sync(0xffffffffu, tile, 0);
+      if (tile >= p.total_tiles) break;
+      const TileInfo ti = decode_tile(p, tile);
+      const gwsig_problem& P = p.prob[ti.prob];
+      const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
+      const int m0 = ti.tm * BM, n0 = ti.tn * BN;
+      const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
+      const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
+      const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
+      const bool kmajor = (flags & GWSIG_FLAG_A_KMAJOR) != 0;
+      bool first = true;
+      for (int s = 0; s < nseg; ++s) {
+        const gwsig_seg& S = p.seg[seg_begin + s];
+        const int K = __ldg(&S.K);
+        if (K == 0) continue;
+        const bool last_seg = s == nseg - 1;
+        const gwsig_idx2 ak = S.ak, bk = S.bk;
+        const double2* abase = p.A + __ldg(&S.a_off) + a_boff;
+        const double2* b_col[RB];
+        bool b_ok[RB];
+        {
+          const gwsig_idx2 bn = S.bn;
+          const double2* bbase = p.B + __ldg(&S.b_off) + b_boff;
 #pragma unroll
-    for (int e = 0; e < B_PER; ++e) {
-      int lin = tid + e * NT;
-      b_nl[e] = lin % BN; b_kl[e] = lin / BN;
+          for (int r = 0; r < RB; ++r) {
+            int nl = lane + 32 * r;
+            b_ok[r] = nl < BN && n0 + nl < N;
+            b_col[r] = bbase + (b_ok[r] ? idx2(bn, n0 + nl) : 0);
+          }
+        }
+        auto publish = [&](int k0) {                      // lane 0: slot header, then a releasing arrive
+          if (lane == 0) {
+            SlotHdr& h = hdr[stage];
+            const bool last = last_seg && k0 + BK >= K;
+            h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
+            h.nk4 = (K - k0 > 4) ? 2 : 1;
+            if (first) {
+              TileRec& t = trec[tslot];
+              t.m_rem = M - m0; t.n_rem = N - n0; t.flags = flags; t.m0 = m0; t.n0 = n0;
+              t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
+              t.cm = P.cm; t.cn = P.cn;
+              h.trec = tslot;
+            }
+            mbar_arrive(full0 + 8 * stage);
+          }
+          if (first) { first = false; if (++tslot == STAGES + 1) tslot = 0; }
+        };
+        if (!kmajor) {
+          // ---- A contiguous along m: lane <-> rows lane, lane+32 of the tile ----
+          const gwsig_idx2 am = S.am;
+          const double2* a_row[RA];
+          bool a_ok[RA];
+#pragma unroll
+          for (int r = 0; r < RA; ++r) {
+            int ml = lane + 32 * r;
+            a_ok[r] = ml < BM && m0 + ml < M;
+            a_row[r] = abase + (a_ok[r] ? idx2(am, m0 + ml) : 0);
+          }
+          for (int k0 = 0; k0 < K; k0 += BK) {
+            mbar_wait(empty0 + 8 * stage, phase ^ 1);
+            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
+            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
+#pragma unroll
+            for (int kk = 0; kk < BK; ++kk) {
+              const int k = k0 + kk;
+              const bool kok = k < K;
+              const long long ka = kok ? idx2(ak, k) : 0, kb = kok ? idx2(bk, k) : 0;
+#pragma unroll
+              for (int r = 0; r < RA; ++r)
+                if (lane + 32 * r < BM)
+                  cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, a_row[r] + ka, kok && a_ok[r]);
+#pragma unroll
+              for (int r = 0; r < RB; ++r)
+                if (lane + 32 * r < BN)
+                  cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
+            }
+            mbar_arrive_cp_async(full0 + 8 * stage);
+            publish(k0);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+        } else {
+          // ---- A contiguous along k: lane <-> (k = lane & 7, rows (lane >> 3) + 4 j) ----
+          const gwsig_idx2 am = S.am;
+          const int kl = lane & 7, mr = lane >> 3;
+          int a_roff[RAK];                              // element offsets inside a tile stay < 2^31 (checked by the plan)
+#pragma unroll
+          for (int j = 0; j < RAK; ++j) {
+            int m = m0 + mr + 4 * j;
+            a_roff[j] = m < M ? (int)idx2(am, m) : -1;
+          }
+          for (int k0 = 0; k0 < K; k0 += BK) {
+            mbar_wait(empty0 + 8 * stage, phase ^ 1);
+            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
+            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
+            {
+              const int k = k0 + kl;
+              const bool kok = k < K;
+              const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+              for (int j = 0; j < RAK; ++j) {
+                const bool ok = kok && a_roff[j] >= 0;
+                cp_async16(as + (unsigned)(kl * LDA + mr + 4 * j) * 16u, ok ? ap + a_roff[j] : abase, ok);
+              }
+            }
+#pragma unroll
+            for (int kk = 0; kk < BK; ++kk) {
+              const int k = k0 + kk;
+              const bool kok = k < K;
+              const long long kb = kok ? idx2(bk, k) : 0;
+#pragma unroll
+              for (int r = 0; r < RB; ++r)
+                if (lane + 32 * r < BN)
+                  cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
+            }
+            mbar_arrive_cp_async(full0 + 8 * stage);
+            publish(k0);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+        }
+      }
     }
-
-    // how many 8-row / 8-column MMA sub-tiles of this warp hold real data
-    const int mi_act = min(MI, max(0, (M - m0 - wm0 + 7) >> 3));
-    const int ni_act = min(NI, max(0, (N - n0 - wn0 + 7) >> 3));
-
+    // tell the consumers there is no more work
+    mbar_wait(empty0 + 8 * stage, phase ^ 1);
+    mbar_arrive_cp_async(full0 + 8 * stage);
+    if (lane == 0) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
+    asm volatile("cp.async.wait_all;\n" ::: "memory");
+  } else {
+    // ================================= CONSUMERS ================================================
+    const int wm0 = (warp / WGN) * (MI * 8), wn0 = (warp % WGN) * (NI * 8);
+    const int fr = lane >> 2, fk = lane & 3;         // fragment row / k index of this lane
     double cre[MI][NI][2], cim[MI][NI][2];
-#pragma unroll
-    for (int i = 0; i < MI; ++i)
-#pragma unroll
-      for (int j = 0; j < NI; ++j) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
-
-    // ---- flattened (segment, k0) iteration space; the loader runs STAGES-1 iterations ahead ----
-    const int nseg = P.seg_count;
-    int total_iters = 0;
-    for (int s = 0; s < nseg; ++s) total_iters += (__ldg(&p.seg[P.seg_begin + s].K) + BK - 1) / BK;
-
-    int ld_seg = -1, ld_k0 = 0, ld_K = 0;            // loader position
-    const double2* a_ptr[A_PER];
-    const double2* b_ptr[B_PER];
-    bool a_ok[A_PER], b_ok[B_PER];
-    gwsig_idx2 ak, bk;
-    ak.div = bk.div = GWSIG_NODIV; ak.hi = ak.lo = bk.hi = bk.lo = 0;
-
-    auto next_segment = [&]() {
-      do { ++ld_seg; ld_K = __ldg(&p.seg[P.seg_begin + ld_seg].K); } while (ld_K == 0);   // skip empty segments
-      ld_k0 = 0;
-      const gwsig_seg& S = p.seg[P.seg_begin + ld_seg];
-      ak = S.ak;
-      bk = S.bk;
-#pragma unroll
-      for (int e = 0; e < A_PER; ++e) {
-        int m = m0 + a_ml[e];
-        a_ok[e] = m < M;
-        a_ptr[e] = p.A + S.a_off + a_boff + (a_ok[e] ? idx2(S.am, m) : 0);
-      }
-#pragma unroll
-      for (int e = 0; e < B_PER; ++e) {
-        int n = n0 + b_nl[e];
-        b_ok[e] = n < N;
-        b_ptr[e] = p.B + S.b_off + b_boff + (b_ok[e] ? idx2(S.bn, n) : 0);
-      }
-    };
-
-    auto issue_loads = [&](int stage) {
-      if (ld_seg < 0 || ld_k0 >= ld_K) next_segment();
-      double2* as = As + stage * BK * LDA;
-      double2* bs = Bs + stage * BK * LDB;
-#pragma unroll
-      for (int e = 0; e < A_PER; ++e) {
-        int k = ld_k0 + a_kl[e];
-        bool ok = a_ok[e] && k < ld_K;
-        cp_async16(as + a_kl[e] * LDA + a_ml[e], ok ? (const void*)(a_ptr[e] + idx2(ak, k)) : (const void*)p.A, ok);
-      }
-#pragma unroll
-      for (int e = 0; e < B_PER; ++e) {
-        int k = ld_k0 + b_kl[e];
-        bool ok = b_ok[e] && k < ld_K;
-        cp_async16(bs + b_kl[e] * LDB + b_nl[e], ok ? (const void*)(b_ptr[e] + idx2(bk, k)) : (const void*)p.B, ok);
-      }
-      ld_k0 += BK;
-    };
-
-    int issued = 0;
-#pragma unroll
-    for (int s = 0; s < STAGES - 1; ++s) {
-      if (issued < total_iters) { issue_loads(s); ++issued; }
-      cp_async_commit();
-    }
-
-    for (int it = 0; it < total_iters; ++it) {
-      cp_async_wait<STAGES - 2>();
-      __syncthreads();
-      if (issued < total_iters) { issue_loads((it + STAGES - 1) % STAGES); ++issued; }
-      cp_async_commit();
-
-      const double2* as = As + (it % STAGES) * BK * LDA;
-      const double2* bs = Bs + (it % STAGES) * BK * LDB;
-#pragma unroll
-      for (int kk = 0; kk < BK / 4; ++kk) {
-        double2 af[MI], bf[NI];
+    int tslot = 0;
+    bool active = false, conjA = false, conjB = false;
+    while (true) {
+      mbar_wait(full0 + 8 * stage, phase);
+      const SlotHdr& h = hdr[stage];
+      const int ctl = h.ctl;
+      if (ctl & 4) break;
+      if (ctl & 1) {
+        tslot = h.trec;
+        const TileRec& t = trec[tslot];
+        active = (wm0 < t.m_rem) && (wn0 < t.n_rem);      // warp-uniform: does this warp tile hold data?
+        conjA = (t.flags & GWSIG_FLAG_CONJ_A) != 0; conjB = (t.flags & GWSIG_FLAG_CONJ_B) != 0;
 #pragma unroll
         for (int i = 0; i < MI; ++i)
-          if (i < mi_act) {
-            af[i] = as[(kk * 4 + fk) * LDA + wm0 + i * 8 + fr];
-            if (conjA) af[i].y = -af[i].y;
+#pragma unroll
+          for (int j = 0; j < NI; ++j) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
+      }
+      if (active) {
+        const double2* as = As + stage * BK * LDA + wm0 + fr;
+        const double2* bs = Bs + stage * BK * LDB + wn0 + fr;
+        const int nk4 = h.nk4;
+#pragma unroll
+        for (int kk = 0; kk < BK / 4; ++kk) {
+          if (kk < nk4) {
+            double2 af[MI], bf[NI];
+#pragma unroll
+            for (int i = 0; i < MI; ++i) af[i] = as[(kk * 4 + fk) * LDA + i * 8];
+#pragma unroll
+            for (int j = 0; j < NI; ++j) bf[j] = bs[(kk * 4 + fk) * LDB + j * 8];
+            if (conjA) {
+#pragma unroll
+              for (int i = 0; i < MI; ++i) af[i].y = -af[i].y;
+            }
+            if (conjB) {
+#pragma unroll
+              for (int j = 0; j < NI; ++j) bf[j].y = -bf[j].y;
+            }
+            // four passes over the warp tile: dependent DMMAs are >= MI*NI instructions apart
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+              for (int j = 0; j < NI; ++j) dmma884(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+              for (int j = 0; j < NI; ++j) dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+              for (int j = 0; j < NI; ++j) dmma884(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
+#pragma unroll
+            for (int i = 0; i < MI; ++i) af[i].y = -af[i].y;
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+              for (int j = 0; j < NI; ++j) dmma884(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
           }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+
+      // ---- epilogue after the last slot of a tile: registers -> C (two-level addressing) ----------
+      if ((ctl & 2) && active) {
+        const TileRec& t = trec[tslot];
+        const int m_rem = t.m_rem, n_rem = t.n_rem, m0 = t.m0, n0 = t.n0;
+        const gwsig_idx2 cm = t.cm, cn = t.cn;
+        double2* cbase = p.C + t.c_off;
+        const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
+        long long cn_off[NI][2];
 #pragma unroll
         for (int j = 0; j < NI; ++j)
-          if (j < ni_act) {
-            bf[j] = bs[(kk * 4 + fk) * LDB + wn0 + j * 8 + fr];
-            if (conjB) bf[j].y = -bf[j].y;
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            int nl = wn0 + j * 8 + fk * 2 + c;
+            cn_off[j][c] = nl < n_rem ? idx2(cn, n0 + nl) : -1;
           }
 #pragma unroll
-        for (int i = 0; i < MI; ++i)
-          if (i < mi_act) {
-            const double nai = -af[i].y;
+        for (int i = 0; i < MI; ++i) {
+          int ml = wm0 + i * 8 + fr;
+          if (ml < m_rem) {
+            double2* crow = cbase + idx2(cm, m0 + ml);
 #pragma unroll
             for (int j = 0; j < NI; ++j)
-              if (j < ni_act) {
-                dmma884(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
-                dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
-                dmma884(cre[i][j][0], cre[i][j][1], nai, bf[j].y);
-                dmma884(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
-              }
+#pragma unroll
+              for (int c = 0; c < 2; ++c)
+                if (cn_off[j][c] >= 0) {
+                  double2* dst = crow + cn_off[j][c];
+                  double2 v = make_double2(cre[i][j][c], cim[i][j][c]);
+                  if (accum) { double2 o = *dst; v.x += o.x; v.y += o.y; }
+                  *dst = v;
+                }
           }
+        }
       }
-    }
-    cp_async_wait<0>();
-
-    // ---- epilogue: registers -> C (two-level addressing, optional accumulate) ------------------
-    double2* cbase = p.C + P.c_off + (long long)ti.batch * P.c_bstride + (long long)p.t0 * P.c_tstride;
-    const bool accum = (flags & GWSIG_FLAG_ACCUM) != 0;
-    long long cn_off[NI][2];
-    bool cn_ok[NI][2];
-#pragma unroll
-    for (int j = 0; j < NI; ++j)
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        int n = n0 + wn0 + j * 8 + fk * 2 + c;
-        cn_ok[j][c] = n < N;
-        cn_off[j][c] = cn_ok[j][c] ? idx2(P.cn, n) : 0;
-      }
-#pragma unroll
-    for (int i = 0; i < MI; ++i) {
-      int m = m0 + wm0 + i * 8 + fr;
-      if (m >= M) continue;
-      long long cm_off = idx2(P.cm, m);
-#pragma unroll
-      for (int j = 0; j < NI; ++j)
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-          if (cn_ok[j][c]) {
-            double2* dst = cbase + cm_off + cn_off[j][c];
-            double2 v = make_double2(cre[i][j][c], cim[i][j][c]);
-            if (accum) { double2 o = *dst; v.x += o.x; v.y += o.y; }
-            *dst = v;
-          }
     }
   }
 }
@@ -259,8 +370,7 @@ __global__ void __launch_bounds__(WARPS_M* WARPS_N * 32) zgemm_grouped_dmma(ZgPa
 // ------------------------------------------------------------------------------------------
 // reference engine: same plan, one thread per output element, plain DFMA, no shared memory
 // ------------------------------------------------------------------------------------------
-template <int BM, int BN>
-__global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
+__global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p, int BM, int BN) {
   for (long long tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
     const TileInfo ti = decode_tile(p, tile);
     const gwsig_problem& P = p.prob[ti.prob];
@@ -291,16 +401,18 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
   }
 }
 
-template <int BM, int BN, int WM, int WN, int STAGES>
+template <int MI, int NI, int WGM, int WGN, int STAGES, int MAXREG>
 cudaError_t launch_dmma(const ZgParams& p, int num_sms, cudaStream_t stream) {
-  auto kern = zgemm_grouped_dmma<BM, BN, WM, WN, STAGES>;
+  auto kern = zgemm_grouped_dmma<MI, NI, WGM, WGN, STAGES, MAXREG>;
+  constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
   constexpr int smem = STAGES * 8 * ((BM + 2) + (BN + 2)) * (int)sizeof(double2);
+  constexpr int threads = (WGM * WGN + 1) * 32;
   static bool configured = false;
   static int occ = 1;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WM * WN * 32, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     configured = true;
@@ -308,7 +420,7 @@ cudaError_t launch_dmma(const ZgParams& p, int num_sms, cudaStream_t stream) {
   long long grid = (long long)num_sms * occ;
   if (grid > p.total_tiles) grid = p.total_tiles;
   if (grid < 1) return cudaSuccess;
-  kern<<<(unsigned)grid, WM * WN * 32, smem, stream>>>(p);
+  kern<<<(unsigned)grid, threads, smem, stream>>>(p);
   return cudaGetLastError();
 }
 
@@ -323,12 +435,13 @@ ZgTile zg_tile_shape(int shape_class) {
 
 cudaError_t zg_launch(int engine, int shape_class, const ZgParams& p, int num_sms, cudaStream_t stream) {
   if (p.total_tiles <= 0) return cudaSuccess;
+  const ZgTile ts = zg_tile_shape(shape_class);
   if (engine == 1) {
     long long grid = p.total_tiles < 65535LL * 16 ? p.total_tiles : 65535LL * 16;
-    if (shape_class == 1) zgemm_grouped_reference<64, 32><<<(unsigned)grid, 256, 0, stream>>>(p);
-    else zgemm_grouped_reference<64, 64><<<(unsigned)grid, 256, 0, stream>>>(p);
+    zgemm_grouped_reference<<<(unsigned)grid, 256, 0, stream>>>(p, ts.bm, ts.bn);
     return cudaGetLastError();
   }
-  if (shape_class == 1) return launch_dmma<64, 32, 4, 2, 3>(p, num_sms, stream);
-  return launch_dmma<64, 64, 4, 2, 3>(p, num_sms, stream);
+  // warp tiles 32x16 complex (64 accumulator registers); consumer grid 2x4 (64x64, class 0) or 2x2 (64x32, class 1)
+  if (shape_class == 1) return launch_dmma<4, 2, 2, 2, 4, 128>(p, num_sms, stream);   // 5 warps x 128 regs: 3 CTAs / SM
+  return launch_dmma<4, 2, 2, 4, 4, 112>(p, num_sms, stream);   // 9 warps x 112 regs: 2 CTAs / SM
 }
