@@ -103,6 +103,10 @@ class RandomC1Inputs:
         """V^{k2,k1}_{Q,bj} for every k2 in k2s  [len, naux, nao, nao]"""
         return np.stack([self._V[k2, k1] for k2 in k2s])
 
+    def V1_rows(self, k1: int, k2s) -> np.ndarray:
+        """V^{k1,k2}_{Q,ia} for every k2 in k2s  [len, naux, nao, nao]"""
+        return np.stack([self._V[k1, k2] for k2 in k2s])
+
 
 # ==========================================================================
 # configs 2-5: group-averaged real-space operators
@@ -283,6 +287,15 @@ class SymmetricInputs:
         T = np.tensordot(f2, self.Vd, axes=(0, 1))                   # [nR1, nel]
         f1 = np.exp(-2j * np.pi * (self.kmesh.frac[k2s] @ self.vR1.T))   # [nk2, nR1]
         return (f1 @ T).reshape(len(k2s), self.naux, self.nao, self.nao)
+
+
+    def V1_rows(self, k1: int, k2s) -> np.ndarray:
+        """V^{k1,k2}_{Q,ia} for every k2 in k2s  [len, naux, nao, nao]  (same Bloch sum as V_pair, batched over k2)."""
+        k2s = np.asarray(list(k2s))
+        f1 = np.exp(-2j * np.pi * (self.vR1 @ self.kmesh.frac[k1]))
+        T = np.tensordot(f1, self.Vd, axes=(0, 0))                   # [nR2, nel]
+        f2 = np.exp(+2j * np.pi * (self.kmesh.frac[k2s] @ self.vR2.T))   # [nk2, nR2]
+        return (f2 @ T).reshape(len(k2s), self.naux, self.nao, self.nao)
 
 
 def make_inputs(name: str, **over):

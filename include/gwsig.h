@@ -140,10 +140,23 @@ int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSig
 int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV);
 int gwsig_sigma_end(gwsig_ctx* ctx);
 int gwsig_sigma_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, const void* dW, void* dSigma, void* stream);
+/* sigma_abort : leave an evaluation opened by sigma_begin without writing dSigma (nothing is launched).
+ *               Used to time a prefix of the pair list (bench.py: FULL_BZ on a q subset, scaled).  */
+int gwsig_sigma_abort(gwsig_ctx* ctx);
+/* sigma_eval_host : the same evaluation with HOST buffers (layouts as above; page-locked memory gives
+ *               asynchronous copies, pageable memory works but serialises).  The library owns the
+ *               device side: it copies hG, hW to the device, streams hV through a two-slot device
+ *               ring in batches of whole q (option "v_ring_mib", per slot) on its own copy stream so
+ *               that the transfer of batch n+1 overlaps the contraction of batch n -- "V is copied on
+ *               demand" (Algorithm 4 line 3) -- and copies Sigma back to
+ *               hSigma.  Returns after the result has landed in hSigma (the stream is synchronised). */
+int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, const void* hW, void* hSigma,
+                          void* stream);
 
 /* ---- options and accounting ------------------------------------------------------------------ */
 /* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
- * default 8192), "tau_chunk" (0 = from the budget), "timing" (0/1: record a CUDA event pair around
+ * default 8192), "tau_chunk" (0 = from the budget), "v_ring_mib" (size of one slot of the
+ * V ring of sigma_eval_host, default 1024), "timing" (0/1: record a CUDA event pair around
  * every kernel launch on the launching stream, read back with gwsig_kernel_times)                  */
 int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value);
 /* real flops (8 per complex multiply-add) of one evaluation: the full-BZ dense equivalent
@@ -166,7 +179,8 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
 int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, void* problems_out, void* segs_out);
 
 /* ---- FP64 peak probe (measurement support; needs a device) -------------------------------------
- * kind 0: register-only mma.sync.m8n8k4.f64 issue-rate loop; kind 1: register-only DFMA loop.
+ * kind 0: register-only mma.sync.m8n8k4.f64 issue-rate loop; kind 1: register-only DFMA loop;
+ * kind 2: both interleaved in every warp (tells whether DMMA and DFMA share one pipe).
  * Returns achieved TFLOP/s over `iters` inner iterations on every SM (CUDA-event timed).           */
 int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters,
                      double* tflops, double* ms);

@@ -34,7 +34,7 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_set_symmetry", "gwsig_set_blocks", "gwsig_set_triples", "gwsig_get_ibz", "gwsig_pair_count",
            "gwsig_pair_info", "gwsig_buffer_sizes", "gwsig_sigma_begin", "gwsig_sigma_push_pairs", "gwsig_sigma_end",
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
-           "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times"]
+           "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -49,6 +49,7 @@ _sig = {
     "gwsig_flop_counts": [_vp, _vp, _vp], "gwsig_last_launch_count": [_vp, _vp],
     "gwsig_plan_counts": [_vp, _i64, _i64, _i, _i, _vp, _vp, _vp], "gwsig_plan_get": [_vp, _i64, _i64, _i, _i, _vp, _vp],
     "gwsig_probe_fp64": [_vp, _i, _i, _i, _i64, _vp, _vp], "gwsig_kernel_times": [_vp, _vp, _vp],
+    "gwsig_sigma_abort": [_vp], "gwsig_sigma_eval_host": [_vp, _vp, _vp, _vp, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -204,6 +205,13 @@ class Gwsig:
 
     def sigma_eval(self, dG, dV, dW, dSigma, stream=0):
         self._ck(_lib.gwsig_sigma_eval(self._h, _ptr(dG), _ptr(dV), _ptr(dW), _ptr(dSigma), stream or None))
+
+    def sigma_abort(self):
+        self._ck(_lib.gwsig_sigma_abort(self._h))
+
+    def sigma_eval_host(self, hG, hV, hW, hSigma, stream=0):
+        """host buffers (numpy arrays or pinned CPU torch tensors); blocks until hSigma holds the result."""
+        self._ck(_lib.gwsig_sigma_eval_host(self._h, _ptr(hG), _ptr(hV), _ptr(hW), _ptr(hSigma), stream or None))
 
     def probe_fp64(self, kind, warps_per_block=8, blocks_per_sm=2, iters=20000):
         t, ms = C.c_double(), C.c_double()

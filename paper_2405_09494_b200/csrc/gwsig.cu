@@ -61,6 +61,7 @@ struct gwsig_ctx {
   int engine = GWSIG_ENGINE_DMMA;
   int hermitize = 0;
   long long scratch_mib = 8192;
+  long long v_ring_mib = 1024;
   int tau_chunk = 0;
   // evaluation state
   bool in_eval = false;
@@ -72,6 +73,9 @@ struct gwsig_ctx {
   long long launches = 0;
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
+  DevBuf h_g, h_w, h_sig, h_vslot[2];           // device side of sigma_eval_host
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_freed[2] = {nullptr, nullptr};
   DevBuf tgt_src, tgt_op, colphase_ao, ell_cols_ao, ell_vals_ao, ell_cnt_ao;     // unfold tables (ao)
   DevBuf wtgt_src, wtgt_op, colphase_aux, ell_cols_aux, ell_vals_aux, ell_cnt_aux;
   int maxnz_ao = 0, maxnz_aux = 0;
@@ -295,8 +299,15 @@ int gwsig_destroy(gwsig_ctx* ctx) {
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
                       &ctx->probe_sink, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
-                      &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux};
+                      &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
+                      &ctx->h_vslot[0], &ctx->h_vslot[1]};
     for (DevBuf* b : bufs) b->release();
+    for (int i = 0; i < 2; ++i) {
+      if (ctx->ev_copied[i]) cudaEventDestroy(ctx->ev_copied[i]);
+      if (ctx->ev_freed[i]) cudaEventDestroy(ctx->ev_freed[i]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     for (auto& kv : ctx->plan_cache)
       for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); }
   }
@@ -409,6 +420,7 @@ int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
     ctx->engine = (int)value;
   } else if (k == "hermitize") ctx->hermitize = value != 0;
   else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
+  else if (k == "v_ring_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: v_ring_mib < 1"); ctx->v_ring_mib = value; }
   else if (k == "timing") ctx->timing = value != 0;
   else if (k == "tau_chunk") { if (value < 0) return fail(ctx, GWSIG_ERR_ARG, "set_option: tau_chunk < 0"); ctx->tau_chunk = (int)value; }
   else return fail(ctx, GWSIG_ERR_ARG, "set_option: unknown key " + k);
@@ -615,9 +627,71 @@ int gwsig_sigma_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, const v
   return gwsig_sigma_end(ctx);
 }
 
+int gwsig_sigma_abort(gwsig_ctx* ctx) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  if (!ctx->in_eval) return fail(ctx, GWSIG_ERR_ORDER, "sigma_abort: no evaluation is open");
+  ctx->in_eval = false;
+  return GWSIG_OK;
+}
+
+int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, const void* hW, void* hSigma, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "sigma_eval_host: plan incomplete (set_symmetry / set_triples)");
+  if (!hG || !hV_all || !hW || !hSigma) return fail(ctx, GWSIG_ERR_ARG, "sigma_eval_host: NULL host pointer");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!ctx->copy_stream) {
+    CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CU(cudaEventCreateWithFlags(&ctx->ev_copied[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&ctx->ev_freed[i], cudaEventDisableTiming));
+    }
+  }
+  const size_t cb = sizeof(double2);
+  CU(ctx->h_g.ensure(std::max<size_t>(P.g_elems * cb, 16)));
+  CU(ctx->h_w.ensure(std::max<size_t>(P.w_elems * cb, 16)));
+  CU(ctx->h_sig.ensure(std::max<size_t>(P.sig_elems * cb, 16)));
+  // batches of whole q (nk1 pairs each) that fit one ring slot; a single q larger than the slot grows the slot
+  const int nk1 = P.nk1;
+  const long long slot_elems_opt = ctx->v_ring_mib * 1048576LL / (long long)cb;
+  std::vector<long long> cuts{0};
+  long long need = 0;
+  for (long long p = 0; p < P.npairs;) {
+    long long e = p + nk1;
+    while (e < P.npairs && P.v_off[e + nk1] - P.v_off[p] <= slot_elems_opt) e += nk1;
+    need = std::max(need, P.v_off[e] - P.v_off[p]);
+    cuts.push_back(e);
+    p = e;
+  }
+  const int nslots = cuts.size() > 2 ? 2 : 1;
+  for (int i = 0; i < nslots; ++i) CU(ctx->h_vslot[i].ensure(std::max<size_t>(need * cb, 16)));
+  CU(cudaMemcpyAsync(ctx->h_g.p, hG, P.g_elems * cb, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(ctx->h_w.p, hW, P.w_elems * cb, cudaMemcpyHostToDevice, st));
+  if ((rc = gwsig_sigma_begin(ctx, ctx->h_g.p, ctx->h_w.p, ctx->h_sig.p, stream))) return rc;
+  const double2* hV = (const double2*)hV_all;
+  for (size_t b = 0; b + 1 < cuts.size(); ++b) {
+    const int slot = (int)(b % nslots);
+    const long long p0 = cuts[b], p1 = cuts[b + 1];
+    if (b >= (size_t)nslots) CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_freed[slot], 0));   // slot consumed?
+    CU(cudaMemcpyAsync(ctx->h_vslot[slot].p, hV + P.v_off[p0], (size_t)(P.v_off[p1] - P.v_off[p0]) * cb, cudaMemcpyHostToDevice,
+                       ctx->copy_stream));
+    CU(cudaEventRecord(ctx->ev_copied[slot], ctx->copy_stream));
+    CU(cudaStreamWaitEvent(st, ctx->ev_copied[slot], 0));
+    if ((rc = gwsig_sigma_push_pairs(ctx, p0, p1 - p0, ctx->h_vslot[slot].p))) { ctx->in_eval = false; return rc; }
+    CU(cudaEventRecord(ctx->ev_freed[slot], st));
+  }
+  if ((rc = gwsig_sigma_end(ctx))) return rc;
+  CU(cudaMemcpyAsync(hSigma, ctx->h_sig.p, P.sig_elems * cb, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return GWSIG_OK;
+}
+
 int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters, double* tflops,
                      double* ms) {
-  if (!ctx || !tflops || warps_per_block < 1 || warps_per_block > 32 || blocks_per_sm < 1 || iters < 1) return GWSIG_ERR_ARG;
+  if (!ctx || !tflops || kind < 0 || kind > 2 || warps_per_block < 1 || warps_per_block > 32 || blocks_per_sm < 1 || iters < 1) return GWSIG_ERR_ARG;
   int rc = ensure_cuda(ctx);
   if (rc) return rc;
   CU(cudaSetDevice(ctx->device));

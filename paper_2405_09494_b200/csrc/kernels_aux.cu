@@ -104,6 +104,28 @@ __global__ void probe_dfma_kernel(long long iters, double* sink) {
   if (s == 123.456) sink[0] = s;
 }
 
+// both pipes' instructions interleaved in every warp: if DMMA and DFMA were separate pipes the sum of the
+// two rates would exceed either probe alone
+template <int NACC>
+__global__ void probe_mixed_kernel(long long iters, double* sink) {
+  double c0[NACC], c1[NACC], c[NACC];
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) { c0[a] = threadIdx.x * 1e-9; c1[a] = a * 1e-9; c[a] = threadIdx.x * 1e-9 + a; }
+  double x = 1.0 + 1e-12 * threadIdx.x, y = 1.0 - 1e-12 * threadIdx.x, z = 1e-9;
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) {
+      dmma884(c0[a], c1[a], x, y);
+#pragma unroll
+      for (int r = 0; r < 8; ++r) c[(a + r) % NACC] = fma(c[(a + r) % NACC], x, z);    // 8 DFMA (256 lane-FMAs) per DMMA (256 FMAs)
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int a = 0; a < NACC; ++a) s += c0[a] + c1[a] + c[a];
+  if (s == 123.456) sink[0] = s;
+}
+
 }  // namespace
 
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream) {
@@ -126,9 +148,12 @@ cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long it
   if (kind == 0) {
     probe_dmma_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
     *flops_out = (double)blocks * warps_per_block * (double)iters * NACC * 512.0;       // 8*8*4*2 per DMMA
-  } else {
+  } else if (kind == 1) {
     probe_dfma_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
     *flops_out = (double)blocks * warps_per_block * 32.0 * (double)iters * NACC * 2.0;
+  } else {
+    probe_mixed_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
+    *flops_out = (double)blocks * warps_per_block * (double)iters * NACC * (512.0 + 8 * 32 * 2.0);
   }
   return cudaGetLastError();
 }
