@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--mode", default="ibz_block", choices=list(MODES))
     ap.add_argument("--no-modes", action="store_true", help="skip the FULL_BZ / IBZ comparison legs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-sample-tau", type=int, default=4, help="tau points of the oracle sample")
     ap.add_argument("--probe-only", action="store_true", help="print the FP64 issue-rate probes and exit")
     return ap.parse_args()
@@ -444,10 +445,11 @@ def main():
                                        "the register-only DMMA probe of this library reaches 36.9 (MEASURED_PEAKS.json has no FP64 entry)"}
 
     # ---- end to end through the host-buffer call ------------------------------------------------------------------
-    et, h2d, d2h, hs = run_e2e(wl, torch, dev, max(1, min(args.steps, 2)), 1)
-    line["e2e"] = {"value": float(np.mean(et)) * 1e3, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                   "api": "gwsig_sigma_eval_host (pinned host G, W, V -> host Sigma; V streamed through a 2-slot ring)"}
-    assert np.abs(hs - sigma_gpu).max() <= 1e-12 * np.abs(sigma_gpu).max(), "host-buffer path disagrees with the resident path"
+    if not args.no_e2e:
+        et, h2d, d2h, hs = run_e2e(wl, torch, dev, max(1, min(args.steps, 2)), 1)
+        line["e2e"] = {"value": float(np.mean(et)) * 1e3, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                       "api": "gwsig_sigma_eval_host (pinned host G, W, V -> host Sigma; V streamed through a 2-slot ring)"}
+        assert np.abs(hs - sigma_gpu).max() <= 1e-12 * np.abs(sigma_gpu).max(), "host-buffer path disagrees with the resident path"
 
     # ---- CPU oracle beside it (baseline, and a live parity sample) ------------------------------------------------
     if not args.no_cpu_baseline:
