@@ -4,10 +4,15 @@
 // arXiv 2405.09494).  Descriptors: include/gwsig_plan.h.  Design: DESIGN.md section 5.
 //
 //  * persistent CTAs, dynamic tile scheduler over a cost-sorted tile list (heaviest problems first)
-//  * warp-specialised: ONE PRODUCER WARP does all index arithmetic (two-level ragged addressing) and
-//    stages operands global -> shared with 16-byte cp.async (one complex128 per copy; ragged edges are
-//    zero-filled), signalling a STAGES-deep ring of mbarriers (cp.async.mbarrier.arrive.noinc);
-//    the CONSUMER WARPS only wait, load fragments and issue DMMA, then release the slot
+//  * warp-specialised, two warpgroups per CTA: FOUR PRODUCER WARPS do all index arithmetic (two-level ragged
+//    addressing) and stage operands global -> shared with 16-byte cp.async (one complex128 per copy; ragged
+//    edges are zero-filled), signalling a STAGES-deep ring of mbarriers (cp.async.mbarrier.arrive.noinc);
+//    the FOUR CONSUMER WARPS only wait, load fragments and issue DMMA, then release the slot.
+//    setmaxnreg moves the producers' registers to the consumers (48 / 208), two CTAs are resident per SM, so
+//    every SM sub-partition holds two consumer warps working on independent tiles (one tile's epilogue
+//    overlaps the other's main loop)
+//  * ragged edges cost no tensor-pipe time: a consumer warp skips the 8-row / 8-column groups of its
+//    warp tile that lie outside the problem
 //  * shared tiles are k-major with leading dimension = 2 (mod 8) complex elements: the
 //    one-double2-per-lane fragment loads of mma.m8n8k4.f64 are bank-conflict free
 //  * complex product = 4 real DMMA per 8x8x4 tile: re += ar*br, im += ar*bi, re += (-ai)*bi, im += ai*br,
@@ -82,9 +87,11 @@ __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long til
 
 // ------------------------------------------------------------------------------------------
 // tensor-core engine, warp-specialised
-//   consumer warps: WGM x WGN, each owning an (8 MI) x (8 NI) complex tile; producer: 1 warp
-//   The producer owns the tile scheduler (one atomicAdd per tile) and every descriptor read; it
-//   tells the consumers what a pipeline slot holds through a small header in shared memory.
+//   consumer warpgroup (warps 0..3): WGM x WGN warps, each owning an (8 MI) x (8 NI) complex tile
+//   producer warpgroup (warps 4..7): owns the tile scheduler (one atomicAdd per tile) and every descriptor
+//   read; tells the consumers what a pipeline slot holds through a small header in shared memory.
+//   Within a slot of BK = 8 k-rows producer warp w stages rows 2w, 2w+1 (A contiguous along m) or the
+//   tile rows = w (mod 4) (A contiguous along k).
 // ------------------------------------------------------------------------------------------
 struct SlotHdr {
   int ctl;            // bit0: first slot of a tile, bit1: last slot of a tile, bit2: no more work
@@ -100,43 +107,59 @@ struct __align__(16) TileRec {   // what the consumers need to know about a tile
   gwsig_idx2 cm, cn;
 };
 
-template <int MI, int NI, int WGM, int WGN, int STAGES, int MAXREG>
-__global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm_grouped_dmma(ZgParams p) {
+constexpr int kProducerWarps = 4;
+constexpr int kProducerRegs = 48;
+constexpr int kConsumerRegs = 208;
+
+__device__ __forceinline__ double flip_sign(double x) {      // integer pipe: keeps the FP64 pipe for DMMA
+  return __hiloint2double(__double2hiint(x) ^ (int)0x80000000, __double2loint(x));
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+template <int MI, int NI, int WGM, int WGN, int STAGES>
+__global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_grouped_dmma(ZgParams p) {
+  static_assert(WGM * WGN == 4, "one consumer warpgroup");
   constexpr int BK = 8;
   constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
   constexpr int NCW = WGM * WGN;                     // consumer warps
   constexpr int LDA = BM + 2, LDB = BN + 2;          // = 2 (mod 8): conflict-free fragment loads
   constexpr int RA = (BM + 31) / 32, RB = (BN + 31) / 32;
-  constexpr int RAK = BM / 4;                        // rows per lane in the k-major A mapping
-  static_assert(LDA % 8 == 2 && LDB % 8 == 2 && BM % 4 == 0, "layout");
+  constexpr int RAK = BM / 16;                       // rows per lane and producer warp in the k-major A mapping
+  static_assert(LDA % 8 == 2 && LDB % 8 == 2 && BM % 16 == 0, "layout");
 
   extern __shared__ double2 zg_smem[];
   double2* As = zg_smem;                             // [STAGES][BK][LDA]
   double2* Bs = zg_smem + STAGES * BK * LDA;         // [STAGES][BK][LDB]
   __shared__ __align__(8) unsigned long long bars[2 * STAGES];
   __shared__ SlotHdr hdr[STAGES];
-  __shared__ TileRec trec[STAGES + 1];        // the producer is at most STAGES tiles ahead of any consumer
+  __shared__ TileRec trec[STAGES + 1];        // the producers are at most STAGES tiles ahead of any consumer
+  __shared__ long long next_tile[2];          // tile id broadcast among the producer warps (double buffered)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
   const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[STAGES]);
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 33); mbar_init(empty0 + 8 * s, NCW); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, kProducerWarps * 32 + 1); mbar_init(empty0 + 8 * s, NCW); }
   }
   __syncthreads();
 
   int stage = 0;
   unsigned phase = 0;
 
-  if (warp == NCW) {
-    // ================================= PRODUCER =================================================
+  if (warp >= NCW) {
+    // ================================= PRODUCERS ================================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kProducerRegs));
+    const int pw = warp - NCW;                          // producer warp 0..3
     const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
-    int tslot = 0;
+    int tslot = 0, tbuf = 0;
     while (true) {
-      long long tile = 0;
-      if (lane == 0) tile = (long long)atomicAdd(p.counter, 1ULL);
-      tile = __shfl_sync(0xffffffffu, tile, 0);
+      if (pw == 0 && lane == 0) next_tile[tbuf] = (long long)atomicAdd(p.counter, 1ULL);
+      named_bar_sync(1, kProducerWarps * 32);
+      const long long tile = next_tile[tbuf];
+      tbuf ^= 1;
       if (tile >= p.total_tiles) break;
       const TileInfo ti = decode_tile(p, tile);
       const gwsig_problem& P = p.prob[ti.prob];
@@ -166,8 +189,8 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
             b_col[r] = bbase + (b_ok[r] ? idx2(bn, n0 + nl) : 0);
           }
         }
-        auto publish = [&](int k0) {                      // lane 0: slot header, then a releasing arrive
-          if (lane == 0) {
+        auto publish = [&](int k0) {                      // producer warp 0, lane 0: slot header, then a releasing arrive
+          if (pw == 0 && lane == 0) {
             SlotHdr& h = hdr[stage];
             const bool last = last_seg && k0 + BK >= K;
             h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
@@ -183,8 +206,22 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
           }
           if (first) { first = false; if (++tslot == STAGES + 1) tslot = 0; }
         };
+        // B rows of this warp: kk = 2 pw, 2 pw + 1 (both A layouts)
+        auto stage_b = [&](int k0, unsigned bs) {
+#pragma unroll
+          for (int h2 = 0; h2 < 2; ++h2) {
+            const int kk = 2 * pw + h2;
+            const int k = k0 + kk;
+            const bool kok = k < K;
+            const long long kb = kok ? idx2(bk, k) : 0;
+#pragma unroll
+            for (int r = 0; r < RB; ++r)
+              if (lane + 32 * r < BN)
+                cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
+          }
+        };
         if (!kmajor) {
-          // ---- A contiguous along m: lane <-> rows lane, lane+32 of the tile ----
+          // ---- A contiguous along m: lane <-> rows lane, lane+32 of the tile; this warp stages k-rows 2 pw, 2 pw + 1 ----
           const gwsig_idx2 am = S.am;
           const double2* a_row[RA];
           bool a_ok[RA];
@@ -199,31 +236,29 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
             const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
             const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
 #pragma unroll
-            for (int kk = 0; kk < BK; ++kk) {
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const int kk = 2 * pw + h2;
               const int k = k0 + kk;
               const bool kok = k < K;
-              const long long ka = kok ? idx2(ak, k) : 0, kb = kok ? idx2(bk, k) : 0;
+              const long long ka = kok ? idx2(ak, k) : 0;
 #pragma unroll
               for (int r = 0; r < RA; ++r)
                 if (lane + 32 * r < BM)
                   cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, a_row[r] + ka, kok && a_ok[r]);
-#pragma unroll
-              for (int r = 0; r < RB; ++r)
-                if (lane + 32 * r < BN)
-                  cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
             }
+            stage_b(k0, bs);
             mbar_arrive_cp_async(full0 + 8 * stage);
             publish(k0);
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
         } else {
-          // ---- A contiguous along k: lane <-> (k = lane & 7, rows (lane >> 3) + 4 j) ----
+          // ---- A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j) ----
           const gwsig_idx2 am = S.am;
-          const int kl = lane & 7, mr = lane >> 3;
+          const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
           int a_roff[RAK];                              // element offsets inside a tile stay < 2^31 (checked by the plan)
 #pragma unroll
           for (int j = 0; j < RAK; ++j) {
-            int m = m0 + mr + 4 * j;
+            int m = m0 + mr + 16 * j;
             a_roff[j] = m < M ? (int)idx2(am, m) : -1;
           }
           for (int k0 = 0; k0 < K; k0 += BK) {
@@ -237,19 +272,10 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
 #pragma unroll
               for (int j = 0; j < RAK; ++j) {
                 const bool ok = kok && a_roff[j] >= 0;
-                cp_async16(as + (unsigned)(kl * LDA + mr + 4 * j) * 16u, ok ? ap + a_roff[j] : abase, ok);
+                cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, ok ? ap + a_roff[j] : abase, ok);
               }
             }
-#pragma unroll
-            for (int kk = 0; kk < BK; ++kk) {
-              const int k = k0 + kk;
-              const bool kok = k < K;
-              const long long kb = kok ? idx2(bk, k) : 0;
-#pragma unroll
-              for (int r = 0; r < RB; ++r)
-                if (lane + 32 * r < BN)
-                  cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
-            }
+            stage_b(k0, bs);
             mbar_arrive_cp_async(full0 + 8 * stage);
             publish(k0);
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -260,15 +286,16 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
     // tell the consumers there is no more work
     mbar_wait(empty0 + 8 * stage, phase ^ 1);
     mbar_arrive_cp_async(full0 + 8 * stage);
-    if (lane == 0) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
+    if (pw == 0 && lane == 0) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
     asm volatile("cp.async.wait_all;\n" ::: "memory");
   } else {
     // ================================= CONSUMERS ================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(kConsumerRegs));
     const int wm0 = (warp / WGN) * (MI * 8), wn0 = (warp % WGN) * (NI * 8);
     const int fr = lane >> 2, fk = lane & 3;         // fragment row / k index of this lane
     double cre[MI][NI][2], cim[MI][NI][2];
-    int tslot = 0;
-    bool active = false, conjA = false, conjB = false;
+    int tslot = 0, mi_eff = 0, ni_eff = 0;           // 8-row / 8-column groups of the warp tile that hold data
+    bool conjA = false, conjB = false;
     while (true) {
       mbar_wait(full0 + 8 * stage, phase);
       const SlotHdr& h = hdr[stage];
@@ -277,14 +304,16 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
       if (ctl & 1) {
         tslot = h.trec;
         const TileRec& t = trec[tslot];
-        active = (wm0 < t.m_rem) && (wn0 < t.n_rem);      // warp-uniform: does this warp tile hold data?
+        mi_eff = min(MI, max(0, (t.m_rem - wm0 + 7) >> 3));
+        ni_eff = min(NI, max(0, (t.n_rem - wn0 + 7) >> 3));
+        if (mi_eff == 0 || ni_eff == 0) mi_eff = ni_eff = 0;
         conjA = (t.flags & GWSIG_FLAG_CONJ_A) != 0; conjB = (t.flags & GWSIG_FLAG_CONJ_B) != 0;
 #pragma unroll
         for (int i = 0; i < MI; ++i)
 #pragma unroll
           for (int j = 0; j < NI; ++j) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
       }
-      if (active) {
+      if (mi_eff > 0) {
         const double2* as = As + stage * BK * LDA + wm0 + fr;
         const double2* bs = Bs + stage * BK * LDB + wn0 + fr;
         const int nk4 = h.nk4;
@@ -292,37 +321,52 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
         for (int kk = 0; kk < BK / 4; ++kk) {
           if (kk < nk4) {
             double2 af[MI], bf[NI];
+            double an[MI];                            // -Im(a) (after the optional conjugation)
 #pragma unroll
-            for (int i = 0; i < MI; ++i) af[i] = as[(kk * 4 + fk) * LDA + i * 8];
+            for (int i = 0; i < MI; ++i)
+              if (i < mi_eff) af[i] = as[(kk * 4 + fk) * LDA + i * 8];
 #pragma unroll
-            for (int j = 0; j < NI; ++j) bf[j] = bs[(kk * 4 + fk) * LDB + j * 8];
-            if (conjA) {
+            for (int j = 0; j < NI; ++j)
+              if (j < ni_eff) bf[j] = bs[(kk * 4 + fk) * LDB + j * 8];
 #pragma unroll
-              for (int i = 0; i < MI; ++i) af[i].y = -af[i].y;
+            for (int i = 0; i < MI; ++i) {
+              const double neg = flip_sign(af[i].y);
+              an[i] = conjA ? af[i].y : neg;
+              af[i].y = conjA ? neg : af[i].y;
             }
             if (conjB) {
 #pragma unroll
-              for (int j = 0; j < NI; ++j) bf[j].y = -bf[j].y;
+              for (int j = 0; j < NI; ++j) bf[j].y = flip_sign(bf[j].y);
             }
-            // four passes over the warp tile: dependent DMMAs are >= MI*NI instructions apart
+            // four passes over the warp tile: dependent DMMAs are >= mi_eff*ni_eff instructions apart
 #pragma unroll
             for (int i = 0; i < MI; ++i)
+              if (i < mi_eff) {
 #pragma unroll
-              for (int j = 0; j < NI; ++j) dmma884(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-#pragma unroll
-              for (int j = 0; j < NI; ++j) dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-#pragma unroll
-              for (int j = 0; j < NI; ++j) dmma884(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
-#pragma unroll
-            for (int i = 0; i < MI; ++i) af[i].y = -af[i].y;
+                for (int j = 0; j < NI; ++j)
+                  if (j < ni_eff) dmma884(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+              }
 #pragma unroll
             for (int i = 0; i < MI; ++i)
+              if (i < mi_eff) {
 #pragma unroll
-              for (int j = 0; j < NI; ++j) dmma884(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
+                for (int j = 0; j < NI; ++j)
+                  if (j < ni_eff) dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+              }
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+              if (i < mi_eff) {
+#pragma unroll
+                for (int j = 0; j < NI; ++j)
+                  if (j < ni_eff) dmma884(cre[i][j][0], cre[i][j][1], an[i], bf[j].y);
+              }
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+              if (i < mi_eff) {
+#pragma unroll
+                for (int j = 0; j < NI; ++j)
+                  if (j < ni_eff) dmma884(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
+              }
           }
         }
       }
@@ -331,7 +375,7 @@ __global__ void __launch_bounds__((WGM* WGN + 1) * 32) __maxnreg__(MAXREG) zgemm
       if (++stage == STAGES) { stage = 0; phase ^= 1; }
 
       // ---- epilogue after the last slot of a tile: registers -> C (two-level addressing) ----------
-      if ((ctl & 2) && active) {
+      if ((ctl & 2) && mi_eff > 0) {
         const TileRec& t = trec[tslot];
         const int m_rem = t.m_rem, n_rem = t.n_rem, m0 = t.m0, n0 = t.n0;
         const gwsig_idx2 cm = t.cm, cn = t.cn;
@@ -401,16 +445,18 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p, int B
   }
 }
 
-template <int MI, int NI, int WGM, int WGN, int STAGES, int MAXREG>
+template <int MI, int NI, int WGM, int WGN, int STAGES>
 cudaError_t launch_dmma(const ZgParams& p, int num_sms, cudaStream_t stream) {
-  auto kern = zgemm_grouped_dmma<MI, NI, WGM, WGN, STAGES, MAXREG>;
+  auto kern = zgemm_grouped_dmma<MI, NI, WGM, WGN, STAGES>;
   constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
   constexpr int smem = STAGES * 8 * ((BM + 2) + (BN + 2)) * (int)sizeof(double2);
-  constexpr int threads = (WGM * WGN + 1) * 32;
+  constexpr int threads = (WGM * WGN + kProducerWarps) * 32;
   static bool configured = false;
   static int occ = 1;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
     if (e != cudaSuccess) return e;
@@ -441,7 +487,8 @@ cudaError_t zg_launch(int engine, int shape_class, const ZgParams& p, int num_sm
     zgemm_grouped_reference<<<(unsigned)grid, 256, 0, stream>>>(p, ts.bm, ts.bn);
     return cudaGetLastError();
   }
-  // warp tiles 32x16 complex (64 accumulator registers); consumer grid 2x4 (64x64, class 0) or 2x2 (64x32, class 1)
-  if (shape_class == 1) return launch_dmma<4, 2, 2, 2, 4, 128>(p, num_sms, stream);   // 5 warps x 128 regs: 3 CTAs / SM
-  return launch_dmma<4, 2, 2, 4, 4, 112>(p, num_sms, stream);   // 9 warps x 112 regs: 2 CTAs / SM
+  // 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 208 / 48 by setmaxnreg.
+  // class 0: warp tiles 32x32 complex (2x2 warps -> 64x64); class 1: warp tiles 32x16 (2x2 warps -> 64x32)
+  if (shape_class == 1) return launch_dmma<4, 2, 2, 2, 6>(p, num_sms, stream);
+  return launch_dmma<4, 4, 2, 2, 5>(p, num_sms, stream);
 }
