@@ -171,7 +171,9 @@ int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
 int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
- * stage: 1 = X = V G, 2 = Y = W X, 3 = Sigma += Y V, 4 = unfold step 1, 5 = unfold step 2.
+ * stage: 1 = X = V G (A = V2, B = G, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
+ * B = W, C = Y), 3 = Sigma += Y V (A = Y, B = V2, C = Sigma accumulator; the segment list of an
+ * output block may be cut into several problems that add into the same C).
  * Descriptors are the structs of include/gwsig_plan.h; offsets are in complex elements relative
  * to the operand bases documented there.                                                           */
 int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, int64_t* nproblems, int64_t* nsegs,

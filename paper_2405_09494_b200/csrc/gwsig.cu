@@ -3,7 +3,7 @@
 //   sigma_begin : [a1] unfold G to the full zone (IBZ mode)            -> Gbz
 //   sigma_push  : [a2] unfold W for the q of the pushed pairs (IBZ)    -> W ring
 //                 per sub-batch of whole q's, per tau chunk:
-//                 [a3] X = conj(V2)^T G, [a4] Y = W^T X, [a5] Sigma_acc += Y V2   (grouped GEMM engine)
+//                 [a3] X = conj(V2)^T G, [a4] Y^T = X^T W, [a5] Sigma_acc += Y V2   (grouped GEMM engine)
 //   sigma_end   : [a6] Sigma = -(1/Nk) Sigma_acc (optional Hermitise)
 #include <cuda_runtime.h>
 
@@ -42,10 +42,9 @@ struct DevBuf {
 };
 
 struct DevStage {
-  DevBuf prob, seg;
+  DevBuf prob, seg, bucket;
   int nprob = 0;
   long long ntiles = 0;
-  int shape_class = 0;
 };
 struct DevPlan { DevStage st[3]; };
 
@@ -225,14 +224,14 @@ int get_dev_plan(gwsig_ctx* ctx, long long p0, long long np, int nt, int q_first
   std::unique_ptr<DevPlan> dp(new DevPlan());
   for (int s = 0; s < 3; ++s) {
     StagePlan sp;
-    int rc = ctx->plan.build_stage(p0, np, nt, s + 1, q_first, sp);
+    int rc = ctx->plan.build_stage(p0, np, nt, s + 1, q_first, sp, ctx->num_sms > 0 ? ctx->num_sms : 148);
     if (rc) return fail(ctx, rc, "internal: build_stage failed");
     DevStage& d = dp->st[s];
     d.nprob = (int)sp.prob.size();
     d.ntiles = sp.ntiles;
-    d.shape_class = sp.shape_class;
     if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
     if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
+    if ((rc = upload(ctx, d.bucket, sp.bucket))) return rc;
   }
   *out = dp.get();
   ctx->plan_cache[key] = std::move(dp);
@@ -268,13 +267,14 @@ int run_stage(gwsig_ctx* ctx, int kind, const DevStage& d, const double2* A, con
   zp.A = A; zp.B = B; zp.C = C;
   zp.prob = (const gwsig_problem*)d.prob.p;
   zp.seg = (const gwsig_seg*)d.seg.p;
+  zp.bucket = (const int*)d.bucket.p;
   zp.nprob = d.nprob;
   zp.total_tiles = d.ntiles;
   zp.t0 = t0;
   zp.counter = (unsigned long long*)ctx->counters.p + ctx->counter_slot++;
   int rc = tic(ctx, kind);
   if (rc) return rc;
-  CU(zg_launch(ctx->engine, d.shape_class, zp, ctx->num_sms, ctx->stream));
+  CU(zg_launch(ctx->engine, zp, ctx->num_sms, ctx->stream));
   if ((rc = toc(ctx))) return rc;
   ctx->launches++;
   return GWSIG_OK;
@@ -309,7 +309,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     for (auto& kv : ctx->plan_cache)
-      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); }
+      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); }
   }
   delete ctx;
   return GWSIG_OK;
@@ -320,7 +320,7 @@ const char* gwsig_last_error(const gwsig_ctx* ctx) { return ctx ? ctx->err.c_str
 static void invalidate(gwsig_ctx* ctx) {
   ctx->tables_ready = false;
   for (auto& kv : ctx->plan_cache)
-    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); }
+    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); }
   ctx->plan_cache.clear();
   ctx->in_eval = false;
 }
@@ -588,7 +588,7 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       int rc = get_dev_plan(ctx, s0, ns, ntc, q_first, &dp);
       if (rc) return rc;
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Vsub, Gsrc, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], Wsrc, (const double2*)ctx->xbuf.p, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
     }
     s0 = s1;

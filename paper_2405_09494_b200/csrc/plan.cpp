@@ -296,8 +296,8 @@ void Plan::w_source(int q, int q_first, long long& off, long long& tstride) cons
 static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo; d.div = GWSIG_NODIV; d.pad_ = 0; return d; }
 static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
 
-int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out) const {
-  out.prob.clear(); out.seg.clear(); out.ntiles = 0; out.shape_class = 0;
+int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out, int num_sms) const {
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0;
   if (p0 < 0 || np < 1 || p0 + np > npairs || nt < 1 || nt > ntau || stage < 1 || stage > 3) return GWSIG_ERR_ARG;
   if (v_off.empty()) return GWSIG_ERR_ARG;
 
@@ -377,16 +377,18 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
           gwsig_seg S; std::memset(&S, 0, sizeof(S));
           gwsig_problem P; std::memset(&P, 0, sizeof(P));
           // Y[P',n](tau) = sum_P W[P,P'](tau) X[P,n](tau)                (Algorithm 4 line 7)
-          S.a_off = woff + blk_off(oq, b);
-          S.am = lvl1(1); S.ak = lvl1(npb);
-          S.b_off = xoff[l] + poff[b];
-          S.bk = lvl1(Np[b]); S.bn = lvl1(1);
+          // lowered TRANSPOSED, Y^T[n,P'] = sum_P X^T[n,P] W[P,P']: the long index n = (iota, alpha, i, b) fills the
+          // 128-row tiles and the ragged block size n_p only meets the 8-column granularity
+          S.a_off = xoff[l] + poff[b];
+          S.am = lvl1(1); S.ak = lvl1(Np[b]);              // A = X^T: m = column of X (contiguous), k = P
+          S.b_off = woff + blk_off(oq, b);
+          S.bk = lvl1(npb); S.bn = lvl1(1);                // B = W[P,P'] row-major
           S.K = npb;
-          P.M = npb; P.N = (int)Np[b];
+          P.M = (int)Np[b]; P.N = npb;
           P.c_off = xoff[l] + poff[b];
-          P.cm = lvl1(Np[b]); P.cn = lvl1(1);
-          P.a_bstride = wts; P.a_tstride = wts;
-          P.b_bstride = xs; P.c_bstride = xs;
+          P.cm = lvl1(1); P.cn = lvl1(Np[b]);              // C = Y^T: element (n, P') at Y[P'][n]
+          P.b_bstride = wts; P.b_tstride = wts;
+          P.a_bstride = xs; P.c_bstride = xs;
           P.nbatch = nt;
           P.flags = 0;
           P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
@@ -398,7 +400,11 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
     // stage 3: Sigma_iota[i,j](tau) += sum over the pairs of this range with the same k1 and their triples
     //          with output block iota of  sum_{P',b} Y[P',i,b] V2[P',b,j]      (Algorithm 4 line 8, PAPER.md:347;
     //          only diagonal (iota,iota) blocks: the others cancel in the q sum -- DESIGN.md A8)
-    int maxN = 0;
+    // split-K: the segment lists are long (all pairs of the range x their triples) and the outputs few and small, so each
+    // problem's list is cut into `parts` pieces of about equal K that add into the same Sigma block (FP64 atomics)
+    struct P3 { gwsig_problem P; std::vector<gwsig_seg> segs; long long kt; };
+    std::vector<P3> p3;
+    long long tiles1 = 0;
     for (int i1 = 0; i1 < nk1; ++i1) {
       const int k1 = out_list[i1];
       const std::vector<int>& o1 = ao_off[k1];
@@ -428,40 +434,89 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
       for (int b = 0; b < nb1; ++b) {
         if (segs[b].empty()) continue;
         const int ni = o1[b + 1] - o1[b];
-        gwsig_problem P; std::memset(&P, 0, sizeof(P));
-        P.M = nt * ni; P.N = ni;
-        P.c_off = sig_off[i1] + blk_off(o1, b);
-        P.cm = lvl2(ni, sts, ni); P.cn = lvl1(1);
-        P.c_tstride = sts;
-        P.nbatch = 1;
-        P.flags = GWSIG_FLAG_ACCUM | GWSIG_FLAG_A_KMAJOR;
-        P.seg_begin = (int)out.seg.size(); P.seg_count = (int)segs[b].size();
-        long long kt = 0;
-        for (auto& S : segs[b]) { out.seg.push_back(S); kt += S.K; }
-        out.prob.push_back(P); cost.push_back(kt);
-        maxN = std::max(maxN, ni);
+        P3 x;
+        std::memset(&x.P, 0, sizeof(x.P));
+        x.P.M = nt * ni; x.P.N = ni;
+        x.P.c_off = sig_off[i1] + blk_off(o1, b);
+        x.P.cm = lvl2(ni, sts, ni); x.P.cn = lvl1(1);
+        x.P.c_tstride = sts;
+        x.P.nbatch = 1;
+        x.P.flags = GWSIG_FLAG_ACCUM | GWSIG_FLAG_A_KMAJOR;
+        x.kt = 0;
+        for (auto& S : segs[b]) x.kt += S.K;
+        x.segs.swap(segs[b]);
+        tiles1 += (long long)zg_tiles_m(x.P.M) * zg_tiles_n(x.P.N);
+        p3.push_back(std::move(x));
       }
     }
-    out.shape_class = maxN <= 32 ? 1 : 0;
+    // enough tiles for ~6 rounds of 2 CTAs per SM, pieces of at least ~512 k
+    const long long want = 12LL * std::max(num_sms, 1);
+    for (auto& x : p3) {
+      long long parts = tiles1 > 0 ? (want + tiles1 - 1) / tiles1 : 1;
+      parts = std::max(1LL, std::min<long long>(parts, std::max(1LL, x.kt / 512)));
+      if ((long long)x.segs.size() < parts) {
+        // too few segments to deal out: cut every segment along P' (k = (P', b): both operands advance by N_p per P')
+        const long long r = (parts + (long long)x.segs.size() - 1) / (long long)x.segs.size();
+        std::vector<gwsig_seg> cut;
+        for (const auto& S : x.segs) {
+          const int na = S.ak.div, npp = S.K / na;
+          const long long pieces = std::min<long long>(r, npp);
+          for (long long c = 0; c < pieces; ++c) {
+            const int P0 = (int)(npp * c / pieces), P1 = (int)(npp * (c + 1) / pieces);
+            gwsig_seg Sc = S;
+            Sc.a_off += (long long)P0 * S.ak.hi;
+            Sc.b_off += (long long)P0 * S.bk.hi;
+            Sc.K = (P1 - P0) * na;
+            cut.push_back(Sc);
+          }
+        }
+        x.segs.swap(cut);
+      }
+      parts = std::min<long long>(parts, (long long)x.segs.size());
+      size_t s0 = 0;
+      long long kdone = 0;
+      for (long long part = 0; part < parts; ++part) {
+        const long long target = x.kt * (part + 1) / parts;
+        gwsig_problem P = x.P;
+        P.seg_begin = (int)out.seg.size();
+        long long kt = 0;
+        while (s0 < x.segs.size() && (kdone < target || part == parts - 1)) {
+          out.seg.push_back(x.segs[s0]);
+          kdone += x.segs[s0].K; kt += x.segs[s0].K;
+          ++s0;
+        }
+        P.seg_count = (int)out.seg.size() - P.seg_begin;
+        if (P.seg_count == 0) continue;
+        out.prob.push_back(P); cost.push_back(kt);
+      }
+    }
   }
 
-  // heaviest problems first (dynamic scheduler takes tiles in order), then the tile prefix
+  // heaviest problems first (dynamic scheduler takes tiles in order), then the tile prefix and the bucket table
   std::vector<int> order(out.prob.size());
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost[x] > cost[y]; });
   std::vector<gwsig_problem> sorted(out.prob.size());
-  const ZgTile ts = zg_tile_shape(out.shape_class);
   long long tb = 0;
   for (size_t i = 0; i < order.size(); ++i) {
     gwsig_problem P = out.prob[order[i]];
-    P.tiles_m = (P.M + ts.bm - 1) / ts.bm;
-    P.tiles_n = (P.N + ts.bn - 1) / ts.bn;
+    P.tiles_m = zg_tiles_m(P.M);
+    P.tiles_n = zg_tiles_n(P.N);
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
     sorted[i] = P;
   }
   out.prob.swap(sorted);
   out.ntiles = tb;
+  out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
+  {
+    size_t pi = 0;
+    for (size_t bkt = 0; bkt < out.bucket.size(); ++bkt) {
+      const long long t = (long long)bkt << ZG_BUCKET_SHIFT;
+      while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
+      out.bucket[bkt] = (int)pi;
+    }
+  }
   return GWSIG_OK;
 }
 

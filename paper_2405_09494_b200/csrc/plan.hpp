@@ -17,8 +17,8 @@ typedef std::complex<double> cplx;
 struct StagePlan {
   std::vector<gwsig_problem> prob;
   std::vector<gwsig_seg> seg;
+  std::vector<int> bucket;    // bucket[t >> 6] = problem holding tile (t & ~63)   (zgemm_grouped.cuh)
   long long ntiles = 0;
-  int shape_class = 0;
 };
 
 struct Plan {
@@ -95,7 +95,9 @@ struct Plan {
   void w_source(int q, int q_first, long long& off, long long& tstride) const;
 
   // lowering to descriptors; stage 1..3 as in gwsig_plan_get()
-  int build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out) const;
+  // split_k > 1 cuts the segment list of every stage-3 problem into that many parts (separate problems that add
+  // into the same Sigma block); 0 = choose so that the launch has enough tiles for `num_sms` SMs
+  int build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out, int num_sms = 148) const;
   void flop_counts(double& full_equiv, double& executed) const;
 };
 

@@ -1,22 +1,24 @@
-// Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a).
+// Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a), engine v3.
 //
 // Serves the three contraction stages of the GW self-energy (Algorithm 4 lines 5, 7, 8 of
 // arXiv 2405.09494).  Descriptors: include/gwsig_plan.h.  Design: DESIGN.md section 5.
 //
-//  * persistent CTAs, dynamic tile scheduler over a cost-sorted tile list (heaviest problems first)
-//  * warp-specialised, two warpgroups per CTA: FOUR PRODUCER WARPS do all index arithmetic (two-level ragged
-//    addressing) and stage operands global -> shared with 16-byte cp.async (one complex128 per copy; ragged
-//    edges are zero-filled), signalling a STAGES-deep ring of mbarriers (cp.async.mbarrier.arrive.noinc);
-//    the FOUR CONSUMER WARPS only wait, load fragments and issue DMMA, then release the slot.
-//    setmaxnreg moves the producers' registers to the consumers (48 / 208), two CTAs are resident per SM, so
-//    every SM sub-partition holds two consumer warps working on independent tiles (one tile's epilogue
-//    overlaps the other's main loop)
-//  * ragged edges cost no tensor-pipe time: a consumer warp skips the 8-row / 8-column groups of its
-//    warp tile that lie outside the problem
+//  * persistent CTAs (2 per SM), dynamic tile scheduler over a cost-sorted tile list; the tile counter is
+//    fetched one tile ahead and a tile is mapped to its problem through a 64-tile bucket table
+//  * warp-specialised: FOUR PRODUCER WARPS do all index arithmetic (two-level ragged addressing) and stage
+//    operands global -> shared with 16-byte cp.async (one complex128 per copy), signalling a STAGES-deep ring
+//    of mbarriers (cp.async.mbarrier.arrive.noinc); the FOUR CONSUMER WARPS only wait, load fragments and
+//    issue DMMA, then release the slot.  setmaxnreg moves the producers' registers to the consumers.
+//  * tile = 128 rows x (<= 4 column groups of 8).  The 16 row groups of a tile are dealt round-robin to the
+//    four consumer warps (warp w owns groups w, w+4, w+8, w+12), every warp owns all column groups: ragged
+//    edges leave no warp idle, and the main loop is instantiated for every (row groups, column groups) count
+//    of a warp -- 16 variants of straight-line, unpredicated DMMA -- so padding never reaches the tensor pipe
+//    beyond the last group of 8 (rows, columns) or 4 (k)
 //  * shared tiles are k-major with leading dimension = 2 (mod 8) complex elements: the
 //    one-double2-per-lane fragment loads of mma.m8n8k4.f64 are bank-conflict free
 //  * complex product = 4 real DMMA per 8x8x4 tile: re += ar*br, im += ar*bi, re += (-ai)*bi, im += ai*br,
-//    issued in two passes over the warp tile so that dependent DMMAs are MI*NI*2 instructions apart
+//    issued in four passes over the warp tile so that dependent DMMAs are far apart
+//  * GWSIG_FLAG_ACCUM tiles add into C with red.global.add.f64 (split-K parts of stage 3 share a Sigma block)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -61,17 +63,23 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
+__device__ __forceinline__ double xor_hi(double x, unsigned m) {      // sign flips on the integer pipe
+  return __hiloint2double(__double2hiint(x) ^ (int)m, __double2loint(x));
+}
+__device__ __forceinline__ void red_add(double* addr, double v) {
+  asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(addr), "d"(v) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
+}
 
-// linear tile id -> problem (binary search on tile_begin), batch entry, tile coordinates
+// linear tile id -> problem (bucket table + short forward scan on tile_begin), batch entry, tile coordinates
 struct TileInfo {
   int prob, batch, tm, tn;
 };
 __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long tile) {
-  int lo = 0, hi = p.nprob - 1;
-  while (lo < hi) {
-    int mid = (lo + hi + 1) >> 1;
-    if (__ldg(&p.prob[mid].tile_begin) <= tile) lo = mid; else hi = mid - 1;
-  }
+  int lo = __ldg(&p.bucket[tile >> ZG_BUCKET_SHIFT]);
+  while (lo + 1 < p.nprob && __ldg(&p.prob[lo + 1].tile_begin) <= tile) ++lo;
   const gwsig_problem& P = p.prob[lo];
   long long local = tile - __ldg(&P.tile_begin);
   int tn_ = __ldg(&P.tiles_n);
@@ -85,14 +93,6 @@ __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long til
   return t;
 }
 
-// ------------------------------------------------------------------------------------------
-// tensor-core engine, warp-specialised
-//   consumer warpgroup (warps 0..3): WGM x WGN warps, each owning an (8 MI) x (8 NI) complex tile
-//   producer warpgroup (warps 4..7): owns the tile scheduler (one atomicAdd per tile) and every descriptor
-//   read; tells the consumers what a pipeline slot holds through a small header in shared memory.
-//   Within a slot of BK = 8 k-rows producer warp w stages rows 2w, 2w+1 (A contiguous along m) or the
-//   tile rows = w (mod 4) (A contiguous along k).
-// ------------------------------------------------------------------------------------------
 struct SlotHdr {
   int ctl;            // bit0: first slot of a tile, bit1: last slot of a tile, bit2: no more work
   int nk4;            // k4-steps of this slot that hold data (1 or 2)
@@ -100,7 +100,7 @@ struct SlotHdr {
   int pad_;
 };
 struct __align__(16) TileRec {   // what the consumers need to know about a tile (written by the producer)
-  int m_rem, n_rem;   // M - m0, N - n0
+  int mrows, ncols;   // rows / columns of this tile that exist
   int flags, pad_;
   long long c_off;    // element offset of C(m = 0, n = 0) incl. batch / tau offsets
   int m0, n0;
@@ -108,63 +108,151 @@ struct __align__(16) TileRec {   // what the consumers need to know about a tile
 };
 
 constexpr int kProducerWarps = 4;
-constexpr int kProducerRegs = 48;
-constexpr int kConsumerRegs = 208;
+constexpr int kConsumerWarps = 4;
+constexpr int kProducerRegs = 56;
+constexpr int kConsumerRegs = 200;
+constexpr int BK = 8;
+constexpr int LDA = ZG_BM + 2, LDB = ZG_BN + 2;          // = 2 (mod 8): conflict-free fragment loads
+constexpr int kStages = 5;
+static_assert(LDA % 8 == 2 && LDB % 8 == 2, "layout");
 
-__device__ __forceinline__ double flip_sign(double x) {      // integer pipe: keeps the FP64 pipe for DMMA
-  return __hiloint2double(__double2hiint(x) ^ (int)0x80000000, __double2loint(x));
+// ------------------------------------------------------------------------------------------
+// consumer side: one warp tile = MI row groups (8 rows each, 32 rows apart) x NI column groups, accumulators
+// acc[i][j] = {re(c0), re(c1), im(c0), im(c1)} of the 8x8 DMMA tile (i, j)
+// ------------------------------------------------------------------------------------------
+template <int MI, int NI>
+__device__ __forceinline__ void consume_k4(double (&acc)[4][4][4], const double2* as, const double2* bs, unsigned mask_n,
+                                           unsigned mask_y, unsigned mask_b) {
+  double2 af[MI], bf[NI];
+  double an[MI];                              // -Im(a) (after the optional conjugation)
+#pragma unroll
+  for (int i = 0; i < MI; ++i) af[i] = as[i * 32];
+#pragma unroll
+  for (int j = 0; j < NI; ++j) bf[j] = bs[j * 8];
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    an[i] = xor_hi(af[i].y, mask_n);
+    af[i].y = xor_hi(af[i].y, mask_y);
+  }
+  if (mask_b) {
+#pragma unroll
+    for (int j = 0; j < NI; ++j) bf[j].y = xor_hi(bf[j].y, mask_b);
+  }
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i].x, bf[j].x);
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][2], acc[i][j][3], af[i].x, bf[j].y);
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], an[i], bf[j].y);
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][2], acc[i][j][3], af[i].y, bf[j].x);
 }
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
+
+template <int MI, int NI>
+__device__ __forceinline__ void consume_slot(double (&acc)[4][4][4], const double2* as, const double2* bs, int nk4,
+                                             unsigned mask_n, unsigned mask_y, unsigned mask_b) {
+  consume_k4<MI, NI>(acc, as, bs, mask_n, mask_y, mask_b);
+  if (nk4 > 1) consume_k4<MI, NI>(acc, as + 4 * LDA, bs + 4 * LDB, mask_n, mask_y, mask_b);
 }
 
-template <int MI, int NI, int WGM, int WGN, int STAGES>
-__global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_grouped_dmma(ZgParams p) {
-  static_assert(WGM * WGN == 4, "one consumer warpgroup");
-  constexpr int BK = 8;
-  constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
-  constexpr int NCW = WGM * WGN;                     // consumer warps
-  constexpr int LDA = BM + 2, LDB = BN + 2;          // = 2 (mod 8): conflict-free fragment loads
-  constexpr int RA = (BM + 31) / 32, RB = (BN + 31) / 32;
-  constexpr int RAK = BM / 16;                       // rows per lane and producer warp in the k-major A mapping
-  static_assert(LDA % 8 == 2 && LDB % 8 == 2 && BM % 16 == 0, "layout");
+// registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + 2 fk + c of the tile
+template <int MI, int NI>
+__device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const TileRec& t, double2* C, int warp, int fr, int fk) {
+  const int mrows = t.mrows, ncols = t.ncols, m0 = t.m0, n0 = t.n0;
+  const gwsig_idx2 cm = t.cm, cn = t.cn;
+  double2* cbase = C + t.c_off;
+  const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
+  long long cn_off[NI][2];
+#pragma unroll
+  for (int j = 0; j < NI; ++j)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int nl = j * 8 + fk * 2 + c;
+      cn_off[j][c] = nl < ncols ? idx2(cn, n0 + nl) : -1;
+    }
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    const int ml = (warp + 4 * i) * 8 + fr;
+    if (ml < mrows) {
+      double2* crow = cbase + idx2(cm, m0 + ml);
+#pragma unroll
+      for (int j = 0; j < NI; ++j)
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          if (cn_off[j][c] >= 0) {
+            double2* dst = crow + cn_off[j][c];
+            if (accum) {
+              red_add(&dst->x, acc[i][j][c]);
+              red_add(&dst->y, acc[i][j][2 + c]);
+            } else {
+              *dst = make_double2(acc[i][j][c], acc[i][j][2 + c]);
+            }
+          }
+    }
+  }
+}
 
+#define ZG_VARIANTS(F)                                                                                   \
+  case 0: F(1, 1) break;  case 1: F(1, 2) break;  case 2: F(1, 3) break;  case 3: F(1, 4) break;       \
+  case 4: F(2, 1) break;  case 5: F(2, 2) break;  case 6: F(2, 3) break;  case 7: F(2, 4) break;       \
+  case 8: F(3, 1) break;  case 9: F(3, 2) break;  case 10: F(3, 3) break; case 11: F(3, 4) break;      \
+  case 12: F(4, 1) break; case 13: F(4, 2) break; case 14: F(4, 3) break; case 15: F(4, 4) break;
+
+// ------------------------------------------------------------------------------------------
+// the kernel: warps 0..3 consume, warps 4..7 produce
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zgemm_grouped_dmma(ZgParams p) {
   extern __shared__ double2 zg_smem[];
-  double2* As = zg_smem;                             // [STAGES][BK][LDA]
-  double2* Bs = zg_smem + STAGES * BK * LDA;         // [STAGES][BK][LDB]
-  __shared__ __align__(8) unsigned long long bars[2 * STAGES];
-  __shared__ SlotHdr hdr[STAGES];
-  __shared__ TileRec trec[STAGES + 1];        // the producers are at most STAGES tiles ahead of any consumer
+  double2* As = zg_smem;                             // [kStages][BK][LDA]
+  double2* Bs = zg_smem + kStages * BK * LDA;        // [kStages][BK][LDB]
+  __shared__ __align__(8) unsigned long long bars[2 * kStages];
+  __shared__ SlotHdr hdr[kStages];
+  __shared__ TileRec trec[kStages + 1];       // the producers are at most kStages tiles ahead of any consumer
   __shared__ long long next_tile[2];          // tile id broadcast among the producer warps (double buffered)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
-  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[STAGES]);
+  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[kStages]);
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, kProducerWarps * 32 + 1); mbar_init(empty0 + 8 * s, NCW); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, kProducerWarps * 32 + 1); mbar_init(empty0 + 8 * s, kConsumerWarps); }
   }
   __syncthreads();
 
   int stage = 0;
   unsigned phase = 0;
 
-  if (warp >= NCW) {
+  if (warp >= kConsumerWarps) {
     // ================================= PRODUCERS ================================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kProducerRegs));
-    const int pw = warp - NCW;                          // producer warp 0..3
+    const int pw = warp - kConsumerWarps;               // producer warp 0..3
+    const bool leader = pw == 0 && lane == 0;
     const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
     int tslot = 0, tbuf = 0;
+    long long pre = 0;                                  // tile id fetched one tile ahead (leader only)
+    if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);
     while (true) {
-      if (pw == 0 && lane == 0) next_tile[tbuf] = (long long)atomicAdd(p.counter, 1ULL);
+      if (leader) next_tile[tbuf] = pre;
       named_bar_sync(1, kProducerWarps * 32);
       const long long tile = next_tile[tbuf];
       tbuf ^= 1;
       if (tile >= p.total_tiles) break;
+      if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);       // lands while this tile is being staged
       const TileInfo ti = decode_tile(p, tile);
       const gwsig_problem& P = p.prob[ti.prob];
       const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
-      const int m0 = ti.tm * BM, n0 = ti.tn * BN;
+      const int m0 = ti.tm * ZG_BM;
+      int n0, ncols;
+      zg_ntile(N, __ldg(&P.tiles_n), ti.tn, n0, ncols);
+      const int mrows = min(ZG_BM, M - m0);
       const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
       const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
       const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
@@ -177,59 +265,47 @@ __global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_gro
         const bool last_seg = s == nseg - 1;
         const gwsig_idx2 ak = S.ak, bk = S.bk;
         const double2* abase = p.A + __ldg(&S.a_off) + a_boff;
-        const double2* b_col[RB];
-        bool b_ok[RB];
-        {
-          const gwsig_idx2 bn = S.bn;
-          const double2* bbase = p.B + __ldg(&S.b_off) + b_boff;
-#pragma unroll
-          for (int r = 0; r < RB; ++r) {
-            int nl = lane + 32 * r;
-            b_ok[r] = nl < BN && n0 + nl < N;
-            b_col[r] = bbase + (b_ok[r] ? idx2(bn, n0 + nl) : 0);
-          }
-        }
-        auto publish = [&](int k0) {                      // producer warp 0, lane 0: slot header, then a releasing arrive
-          if (pw == 0 && lane == 0) {
+        const bool b_ok = lane < ncols;
+        const double2* b_col = p.B + __ldg(&S.b_off) + b_boff + (b_ok ? idx2(S.bn, n0 + lane) : 0);
+        auto publish = [&](int k0) {                      // leader: slot header, then a releasing arrive
+          if (leader) {
             SlotHdr& h = hdr[stage];
             const bool last = last_seg && k0 + BK >= K;
             h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
             h.nk4 = (K - k0 > 4) ? 2 : 1;
             if (first) {
               TileRec& t = trec[tslot];
-              t.m_rem = M - m0; t.n_rem = N - n0; t.flags = flags; t.m0 = m0; t.n0 = n0;
+              t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
               t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
               t.cm = P.cm; t.cn = P.cn;
               h.trec = tslot;
             }
             mbar_arrive(full0 + 8 * stage);
           }
-          if (first) { first = false; if (++tslot == STAGES + 1) tslot = 0; }
+          if (first) { first = false; if (++tslot == kStages + 1) tslot = 0; }
         };
-        // B rows of this warp: kk = 2 pw, 2 pw + 1 (both A layouts)
+        // B rows of this warp: kk = 2 pw, 2 pw + 1 (both A layouts); k-rows beyond the slot's last k4 step are not read
         auto stage_b = [&](int k0, unsigned bs) {
+          if (b_ok) {
 #pragma unroll
-          for (int h2 = 0; h2 < 2; ++h2) {
-            const int kk = 2 * pw + h2;
-            const int k = k0 + kk;
-            const bool kok = k < K;
-            const long long kb = kok ? idx2(bk, k) : 0;
-#pragma unroll
-            for (int r = 0; r < RB; ++r)
-              if (lane + 32 * r < BN)
-                cp_async16(bs + (unsigned)(kk * LDB + lane + 32 * r) * 16u, b_col[r] + kb, kok && b_ok[r]);
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const int kk = 2 * pw + h2;
+              const int k = k0 + kk;
+              if (kk < 4 || k0 + 4 < K) {
+                const bool kok = k < K;
+                cp_async16(bs + (unsigned)(kk * LDB + lane) * 16u, b_col + (kok ? idx2(bk, k) : 0), kok);
+              }
+            }
           }
         };
         if (!kmajor) {
-          // ---- A contiguous along m: lane <-> rows lane, lane+32 of the tile; this warp stages k-rows 2 pw, 2 pw + 1 ----
+          // ---- A contiguous along m: lane <-> rows lane + 32 r of the tile; this warp stages k-rows 2 pw, 2 pw + 1 ----
           const gwsig_idx2 am = S.am;
-          const double2* a_row[RA];
-          bool a_ok[RA];
+          const double2* a_row[4];
 #pragma unroll
-          for (int r = 0; r < RA; ++r) {
-            int ml = lane + 32 * r;
-            a_ok[r] = ml < BM && m0 + ml < M;
-            a_row[r] = abase + (a_ok[r] ? idx2(am, m0 + ml) : 0);
+          for (int r = 0; r < 4; ++r) {
+            const int ml = lane + 32 * r;
+            a_row[r] = ml < mrows ? abase + idx2(am, m0 + ml) : nullptr;
           }
           for (int k0 = 0; k0 < K; k0 += BK) {
             mbar_wait(empty0 + 8 * stage, phase ^ 1);
@@ -239,46 +315,45 @@ __global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_gro
             for (int h2 = 0; h2 < 2; ++h2) {
               const int kk = 2 * pw + h2;
               const int k = k0 + kk;
-              const bool kok = k < K;
-              const long long ka = kok ? idx2(ak, k) : 0;
+              if (kk < 4 || k0 + 4 < K) {
+                const bool kok = k < K;
+                const long long ka = kok ? idx2(ak, k) : 0;
 #pragma unroll
-              for (int r = 0; r < RA; ++r)
-                if (lane + 32 * r < BM)
-                  cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, a_row[r] + ka, kok && a_ok[r]);
-            }
-            stage_b(k0, bs);
-            mbar_arrive_cp_async(full0 + 8 * stage);
-            publish(k0);
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
-          }
-        } else {
-          // ---- A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j) ----
-          const gwsig_idx2 am = S.am;
-          const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
-          int a_roff[RAK];                              // element offsets inside a tile stay < 2^31 (checked by the plan)
-#pragma unroll
-          for (int j = 0; j < RAK; ++j) {
-            int m = m0 + mr + 16 * j;
-            a_roff[j] = m < M ? (int)idx2(am, m) : -1;
-          }
-          for (int k0 = 0; k0 < K; k0 += BK) {
-            mbar_wait(empty0 + 8 * stage, phase ^ 1);
-            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
-            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
-            {
-              const int k = k0 + kl;
-              const bool kok = k < K;
-              const double2* ap = abase + (kok ? idx2(ak, k) : 0);
-#pragma unroll
-              for (int j = 0; j < RAK; ++j) {
-                const bool ok = kok && a_roff[j] >= 0;
-                cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, ok ? ap + a_roff[j] : abase, ok);
+                for (int r = 0; r < 4; ++r)
+                  if (a_row[r]) cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, a_row[r] + ka, kok);
               }
             }
             stage_b(k0, bs);
             mbar_arrive_cp_async(full0 + 8 * stage);
             publish(k0);
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+          }
+        } else {
+          // ---- A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j) ----
+          const gwsig_idx2 am = S.am;
+          const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
+          int a_roff[8];                                // element offsets inside a tile stay < 2^31 (checked by the plan)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int ml = mr + 16 * j;
+            a_roff[j] = ml < mrows ? (int)idx2(am, m0 + ml) : -1;
+          }
+          for (int k0 = 0; k0 < K; k0 += BK) {
+            mbar_wait(empty0 + 8 * stage, phase ^ 1);
+            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
+            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
+            if (kl < 4 || k0 + 4 < K) {
+              const int k = k0 + kl;
+              const bool kok = k < K;
+              const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+              for (int j = 0; j < 8; ++j)
+                if (a_roff[j] >= 0) cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, kok ? ap + a_roff[j] : abase, kok);
+            }
+            stage_b(k0, bs);
+            mbar_arrive_cp_async(full0 + 8 * stage);
+            publish(k0);
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
           }
         }
       }
@@ -286,126 +361,54 @@ __global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_gro
     // tell the consumers there is no more work
     mbar_wait(empty0 + 8 * stage, phase ^ 1);
     mbar_arrive_cp_async(full0 + 8 * stage);
-    if (pw == 0 && lane == 0) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
+    if (leader) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
     asm volatile("cp.async.wait_all;\n" ::: "memory");
   } else {
     // ================================= CONSUMERS ================================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(kConsumerRegs));
-    const int wm0 = (warp / WGN) * (MI * 8), wn0 = (warp % WGN) * (NI * 8);
     const int fr = lane >> 2, fk = lane & 3;         // fragment row / k index of this lane
-    double cre[MI][NI][2], cim[MI][NI][2];
-    int tslot = 0, mi_eff = 0, ni_eff = 0;           // 8-row / 8-column groups of the warp tile that hold data
-    bool conjA = false, conjB = false;
+    double acc[4][4][4];
+    int tslot = 0, variant = -1;
+    unsigned mask_n = 0x80000000u, mask_y = 0, mask_b = 0;
     while (true) {
       mbar_wait(full0 + 8 * stage, phase);
-      const SlotHdr& h = hdr[stage];
-      const int ctl = h.ctl;
+      const int ctl = hdr[stage].ctl;
       if (ctl & 4) break;
       if (ctl & 1) {
-        tslot = h.trec;
+        tslot = hdr[stage].trec;
         const TileRec& t = trec[tslot];
-        mi_eff = min(MI, max(0, (t.m_rem - wm0 + 7) >> 3));
-        ni_eff = min(NI, max(0, (t.n_rem - wn0 + 7) >> 3));
-        if (mi_eff == 0 || ni_eff == 0) mi_eff = ni_eff = 0;
-        conjA = (t.flags & GWSIG_FLAG_CONJ_A) != 0; conjB = (t.flags & GWSIG_FLAG_CONJ_B) != 0;
+        const int mg = (t.mrows + 7) >> 3, ng = (t.ncols + 7) >> 3;
+        const int mi = mg > warp ? (mg - warp + 3) >> 2 : 0;
+        variant = mi > 0 ? (mi - 1) * 4 + (ng - 1) : -1;
+        const bool conjA = (t.flags & GWSIG_FLAG_CONJ_A) != 0;
+        mask_n = conjA ? 0u : 0x80000000u;
+        mask_y = conjA ? 0x80000000u : 0u;
+        mask_b = (t.flags & GWSIG_FLAG_CONJ_B) ? 0x80000000u : 0u;
 #pragma unroll
-        for (int i = 0; i < MI; ++i)
+        for (int i = 0; i < 4; ++i)
 #pragma unroll
-          for (int j = 0; j < NI; ++j) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
+          for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[i][j][c] = 0.0;
       }
-      if (mi_eff > 0) {
-        const double2* as = As + stage * BK * LDA + wm0 + fr;
-        const double2* bs = Bs + stage * BK * LDB + wn0 + fr;
-        const int nk4 = h.nk4;
-#pragma unroll
-        for (int kk = 0; kk < BK / 4; ++kk) {
-          if (kk < nk4) {
-            double2 af[MI], bf[NI];
-            double an[MI];                            // -Im(a) (after the optional conjugation)
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-              if (i < mi_eff) af[i] = as[(kk * 4 + fk) * LDA + i * 8];
-#pragma unroll
-            for (int j = 0; j < NI; ++j)
-              if (j < ni_eff) bf[j] = bs[(kk * 4 + fk) * LDB + j * 8];
-#pragma unroll
-            for (int i = 0; i < MI; ++i) {
-              const double neg = flip_sign(af[i].y);
-              an[i] = conjA ? af[i].y : neg;
-              af[i].y = conjA ? neg : af[i].y;
-            }
-            if (conjB) {
-#pragma unroll
-              for (int j = 0; j < NI; ++j) bf[j].y = flip_sign(bf[j].y);
-            }
-            // four passes over the warp tile: dependent DMMAs are >= mi_eff*ni_eff instructions apart
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-              if (i < mi_eff) {
-#pragma unroll
-                for (int j = 0; j < NI; ++j)
-                  if (j < ni_eff) dmma884(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
-              }
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-              if (i < mi_eff) {
-#pragma unroll
-                for (int j = 0; j < NI; ++j)
-                  if (j < ni_eff) dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
-              }
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-              if (i < mi_eff) {
-#pragma unroll
-                for (int j = 0; j < NI; ++j)
-                  if (j < ni_eff) dmma884(cre[i][j][0], cre[i][j][1], an[i], bf[j].y);
-              }
-#pragma unroll
-            for (int i = 0; i < MI; ++i)
-              if (i < mi_eff) {
-#pragma unroll
-                for (int j = 0; j < NI; ++j)
-                  if (j < ni_eff) dmma884(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
-              }
-          }
-        }
+      if (variant >= 0) {
+        const double2* as = As + stage * BK * LDA + fk * LDA + warp * 8 + fr;
+        const double2* bs = Bs + stage * BK * LDB + fk * LDB + fr;
+        const int nk4 = hdr[stage].nk4;
+#define ZG_F(MI_, NI_) consume_slot<MI_, NI_>(acc, as, bs, nk4, mask_n, mask_y, mask_b);
+        switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
+#undef ZG_F
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+      if (++stage == kStages) { stage = 0; phase ^= 1; }
 
-      // ---- epilogue after the last slot of a tile: registers -> C (two-level addressing) ----------
-      if ((ctl & 2) && mi_eff > 0) {
+      // ---- epilogue after the last slot of a tile ----------
+      if ((ctl & 2) && variant >= 0) {
         const TileRec& t = trec[tslot];
-        const int m_rem = t.m_rem, n_rem = t.n_rem, m0 = t.m0, n0 = t.n0;
-        const gwsig_idx2 cm = t.cm, cn = t.cn;
-        double2* cbase = p.C + t.c_off;
-        const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
-        long long cn_off[NI][2];
-#pragma unroll
-        for (int j = 0; j < NI; ++j)
-#pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            int nl = wn0 + j * 8 + fk * 2 + c;
-            cn_off[j][c] = nl < n_rem ? idx2(cn, n0 + nl) : -1;
-          }
-#pragma unroll
-        for (int i = 0; i < MI; ++i) {
-          int ml = wm0 + i * 8 + fr;
-          if (ml < m_rem) {
-            double2* crow = cbase + idx2(cm, m0 + ml);
-#pragma unroll
-            for (int j = 0; j < NI; ++j)
-#pragma unroll
-              for (int c = 0; c < 2; ++c)
-                if (cn_off[j][c] >= 0) {
-                  double2* dst = crow + cn_off[j][c];
-                  double2 v = make_double2(cre[i][j][c], cim[i][j][c]);
-                  if (accum) { double2 o = *dst; v.x += o.x; v.y += o.y; }
-                  *dst = v;
-                }
-          }
-        }
+#define ZG_F(MI_, NI_) store_tile<MI_, NI_>(acc, t, p.C, warp, fr, fk);
+        switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
+#undef ZG_F
       }
     }
   }
@@ -414,7 +417,7 @@ __global__ void __launch_bounds__((WGM* WGN + kProducerWarps) * 32, 2) zgemm_gro
 // ------------------------------------------------------------------------------------------
 // reference engine: same plan, one thread per output element, plain DFMA, no shared memory
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p, int BM, int BN) {
+__global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
   for (long long tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
     const TileInfo ti = decode_tile(p, tile);
     const gwsig_problem& P = p.prob[ti.prob];
@@ -422,9 +425,11 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p, int B
     const long long a_boff = (long long)ti.batch * P.a_bstride + (long long)p.t0 * P.a_tstride;
     const long long b_boff = (long long)ti.batch * P.b_bstride + (long long)p.t0 * P.b_tstride;
     double2* cbase = p.C + P.c_off + (long long)ti.batch * P.c_bstride + (long long)p.t0 * P.c_tstride;
-    for (int e = threadIdx.x; e < BM * BN; e += blockDim.x) {
-      int m = ti.tm * BM + e / BN, n = ti.tn * BN + e % BN;
-      if (m >= P.M || n >= P.N) continue;
+    int n0, ncols;
+    zg_ntile(P.N, P.tiles_n, ti.tn, n0, ncols);
+    const int m0 = ti.tm * ZG_BM, mrows = min(ZG_BM, P.M - m0);
+    for (int e = threadIdx.x; e < mrows * ncols; e += blockDim.x) {
+      int m = m0 + e / ncols, n = n0 + e % ncols;
       double sr = 0.0, si = 0.0;
       for (int s = 0; s < P.seg_count; ++s) {
         const gwsig_seg& S = p.seg[P.seg_begin + s];
@@ -439,26 +444,32 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p, int B
         }
       }
       double2* dst = cbase + idx2(P.cm, m) + idx2(P.cn, n);
-      if (P.flags & GWSIG_FLAG_ACCUM) { sr += dst->x; si += dst->y; }
-      *dst = make_double2(sr, si);
+      if (P.flags & GWSIG_FLAG_ACCUM) { atomicAdd(&dst->x, sr); atomicAdd(&dst->y, si); }
+      else *dst = make_double2(sr, si);
     }
   }
 }
 
-template <int MI, int NI, int WGM, int WGN, int STAGES>
-cudaError_t launch_dmma(const ZgParams& p, int num_sms, cudaStream_t stream) {
-  auto kern = zgemm_grouped_dmma<MI, NI, WGM, WGN, STAGES>;
-  constexpr int BM = WGM * MI * 8, BN = WGN * NI * 8;
-  constexpr int smem = STAGES * 8 * ((BM + 2) + (BN + 2)) * (int)sizeof(double2);
-  constexpr int threads = (WGM * WGN + kProducerWarps) * 32;
+}  // namespace
+
+cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t stream) {
+  if (p.total_tiles <= 0) return cudaSuccess;
+  if (engine == 1) {
+    long long grid = p.total_tiles < 65535LL * 16 ? p.total_tiles : 65535LL * 16;
+    zgemm_grouped_reference<<<(unsigned)grid, 256, 0, stream>>>(p);
+    return cudaGetLastError();
+  }
+  // 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 200 / 56 by setmaxnreg
+  constexpr int smem = kStages * BK * (LDA + LDB) * (int)sizeof(double2);
+  constexpr int threads = (kConsumerWarps + kProducerWarps) * 32;
   static bool configured = false;
   static int occ = 1;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zgemm_grouped_dmma, threads, smem);
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     configured = true;
@@ -466,29 +477,6 @@ cudaError_t launch_dmma(const ZgParams& p, int num_sms, cudaStream_t stream) {
   long long grid = (long long)num_sms * occ;
   if (grid > p.total_tiles) grid = p.total_tiles;
   if (grid < 1) return cudaSuccess;
-  kern<<<(unsigned)grid, threads, smem, stream>>>(p);
+  zgemm_grouped_dmma<<<(unsigned)grid, threads, smem, stream>>>(p);
   return cudaGetLastError();
-}
-
-}  // namespace
-
-ZgTile zg_tile_shape(int shape_class) {
-  switch (shape_class) {
-    case 1: return ZgTile{64, 32};
-    default: return ZgTile{64, 64};
-  }
-}
-
-cudaError_t zg_launch(int engine, int shape_class, const ZgParams& p, int num_sms, cudaStream_t stream) {
-  if (p.total_tiles <= 0) return cudaSuccess;
-  const ZgTile ts = zg_tile_shape(shape_class);
-  if (engine == 1) {
-    long long grid = p.total_tiles < 65535LL * 16 ? p.total_tiles : 65535LL * 16;
-    zgemm_grouped_reference<<<(unsigned)grid, 256, 0, stream>>>(p, ts.bm, ts.bn);
-    return cudaGetLastError();
-  }
-  // 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 208 / 48 by setmaxnreg.
-  // class 0: warp tiles 32x32 complex (2x2 warps -> 64x64); class 1: warp tiles 32x16 (2x2 warps -> 64x32)
-  if (shape_class == 1) return launch_dmma<4, 2, 2, 2, 6>(p, num_sms, stream);
-  return launch_dmma<4, 4, 2, 2, 5>(p, num_sms, stream);
 }

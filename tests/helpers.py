@@ -122,7 +122,7 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 1)
             run_stage_numpy(pr, sg, Vsub, Gsrc, X, t0)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 2)
-            run_stage_numpy(pr, sg, Wsrc, X, Y, t0)
+            run_stage_numpy(pr, sg, X, Wsrc, Y, t0)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 3)
             run_stage_numpy(pr, sg, Y, Vsub, acc, t0)
         p0 += npp
