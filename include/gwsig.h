@@ -171,7 +171,7 @@ int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
 int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
- * stage: 1 = X = V G (A = V2, B = G, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
+ * stage: 1 = X = V G lowered transposed, X^T = G^T conj(V2) (A = G, B = V2, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
  * B = W, C = Y), 3 = Sigma += Y V (A = Y, B = V2, C = Sigma accumulator; the segment list of an
  * output block may be cut into several problems that add into the same C).
  * Descriptors are the structs of include/gwsig_plan.h; offsets are in complex elements relative

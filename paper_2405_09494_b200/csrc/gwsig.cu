@@ -3,7 +3,7 @@
 //   sigma_begin : [a1] unfold G to the full zone (IBZ mode)            -> Gbz
 //   sigma_push  : [a2] unfold W for the q of the pushed pairs (IBZ)    -> W ring
 //                 per sub-batch of whole q's, per tau chunk:
-//                 [a3] X = conj(V2)^T G, [a4] Y^T = X^T W, [a5] Sigma_acc += Y V2   (grouped GEMM engine)
+//                 [a3] X^T = G^T conj(V2), [a4] Y^T = X^T W, [a5] Sigma_acc += Y V2   (grouped GEMM engine)
 //   sigma_end   : [a6] Sigma = -(1/Nk) Sigma_acc (optional Hermitise)
 #include <cuda_runtime.h>
 
@@ -587,7 +587,7 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       DevPlan* dp = nullptr;
       int rc = get_dev_plan(ctx, s0, ns, ntc, q_first, &dp);
       if (rc) return rc;
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Vsub, Gsrc, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Gsrc, Vsub, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
     }

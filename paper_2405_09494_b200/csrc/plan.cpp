@@ -350,20 +350,22 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
           gwsig_seg S; std::memset(&S, 0, sizeof(S));
           gwsig_problem P; std::memset(&P, 0, sizeof(P));
           // X[P,i,b](tau) = sum_a conj(V2[P,a,i]) G[a,b](tau)          (Algorithm 4 line 5)
-          S.a_off = vrel + L.poff + L.c0;
-          S.am = lvl2(L.ni, L.Np, 1);                     // m = (P, i)
-          S.ak = lvl1(L.ni);                              // k = a
-          S.b_off = goff + blk_off(ao_off[k2], L.al);
-          S.bk = lvl1(L.na);
-          S.bn = lvl2(L.na, gts, 1);                      // n = (tau, b)
+          // lowered TRANSPOSED, X^T[(tau,b),(P,i)] = sum_a G^T[(tau,b),a] conj(V2)[a,(P,i)]: the 8 lanes of a fragment
+          // column then write 8 consecutive b of X (full 128-byte lines) and V2 is the narrow operand
+          S.a_off = goff + blk_off(ao_off[k2], L.al);
+          S.am = lvl2(L.na, gts, 1);                      // m = (tau, b)
+          S.ak = lvl1(L.na);                              // k = a
+          S.b_off = vrel + L.poff + L.c0;
+          S.bk = lvl1(L.ni);
+          S.bn = lvl2(L.ni, L.Np, 1);                     // n = (P, i)
           S.K = L.na;
-          P.M = L.np_ * L.ni; P.N = nt * L.na;
+          P.M = nt * L.na; P.N = L.np_ * L.ni;
           P.c_off = xoff[l] + L.poff + L.c0;
-          P.cm = lvl2(L.ni, L.Np, L.na);
-          P.cn = lvl2(L.na, xs, 1);
-          P.b_tstride = gts;
+          P.cm = lvl2(L.na, xs, 1);
+          P.cn = lvl2(L.ni, L.Np, L.na);
+          P.a_tstride = gts;
           P.nbatch = 1;
-          P.flags = GWSIG_FLAG_CONJ_A;
+          P.flags = GWSIG_FLAG_CONJ_B;
           P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
           out.seg.push_back(S); out.prob.push_back(P); cost.push_back(S.K);
         }

@@ -163,28 +163,28 @@ __device__ __forceinline__ void consume_slot(double (&acc)[4][4][4], const doubl
   if (nk4 > 1) consume_k4<MI, NI>(acc, as + 4 * LDA, bs + 4 * LDB, mask_n, mask_y, mask_b);
 }
 
-// registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + 2 fk + c of the tile
-template <int MI, int NI>
+// registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + 2 fk + c of the tile.
+// One instance for all variants (bounds are run-time, accumulator indices compile-time): keeps the code small.
 __device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const TileRec& t, double2* C, int warp, int fr, int fk) {
   const int mrows = t.mrows, ncols = t.ncols, m0 = t.m0, n0 = t.n0;
   const gwsig_idx2 cm = t.cm, cn = t.cn;
   double2* cbase = C + t.c_off;
   const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
-  long long cn_off[NI][2];
+  long long cn_off[4][2];
 #pragma unroll
-  for (int j = 0; j < NI; ++j)
+  for (int j = 0; j < 4; ++j)
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
       const int nl = j * 8 + fk * 2 + c;
       cn_off[j][c] = nl < ncols ? idx2(cn, n0 + nl) : -1;
     }
 #pragma unroll
-  for (int i = 0; i < MI; ++i) {
+  for (int i = 0; i < 4; ++i) {
     const int ml = (warp + 4 * i) * 8 + fr;
     if (ml < mrows) {
       double2* crow = cbase + idx2(cm, m0 + ml);
 #pragma unroll
-      for (int j = 0; j < NI; ++j)
+      for (int j = 0; j < 4; ++j)
 #pragma unroll
         for (int c = 0; c < 2; ++c)
           if (cn_off[j][c] >= 0) {
@@ -406,9 +406,7 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
       // ---- epilogue after the last slot of a tile ----------
       if ((ctl & 2) && variant >= 0) {
         const TileRec& t = trec[tslot];
-#define ZG_F(MI_, NI_) store_tile<MI_, NI_>(acc, t, p.C, warp, fr, fk);
-        switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
-#undef ZG_F
+        store_tile(acc, t, p.C, warp, fr, fk);
       }
     }
   }

@@ -120,7 +120,7 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
             X = np.zeros(Vsub.size * ntc, complex)
             Y = np.zeros(Vsub.size * ntc, complex)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 1)
-            run_stage_numpy(pr, sg, Vsub, Gsrc, X, t0)
+            run_stage_numpy(pr, sg, Gsrc, Vsub, X, t0)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 2)
             run_stage_numpy(pr, sg, X, Wsrc, Y, t0)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 3)
