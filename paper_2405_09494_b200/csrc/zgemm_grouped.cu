@@ -26,10 +26,15 @@
 
 namespace {
 
+// two-level index: one shared copy of the division code (the kernel's hot code has to stay small: all SMs of a GPC
+// share one instruction cache behind their 32 KB L1.5, and warp-specialised CTAs run several code regions at once)
+__device__ __noinline__ long long idx2_div(long long hi, long long lo, int div, int i) {
+  int q = i / div;
+  return (long long)q * hi + (long long)(i - q * div) * lo;
+}
 __device__ __forceinline__ long long idx2(const gwsig_idx2& d, int i) {
   if (d.div == GWSIG_NODIV) return (long long)i * d.lo;
-  int q = i / d.div;
-  return (long long)q * d.hi + (long long)(i - q * d.div) * d.lo;
+  return idx2_div(d.hi, d.lo, d.div, i);
 }
 
 __device__ __forceinline__ void cp_async16(unsigned smem_dst, const void* gmem_src, bool valid) {
@@ -81,15 +86,15 @@ __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long til
   int lo = __ldg(&p.bucket[tile >> ZG_BUCKET_SHIFT]);
   while (lo + 1 < p.nprob && __ldg(&p.prob[lo + 1].tile_begin) <= tile) ++lo;
   const gwsig_problem& P = p.prob[lo];
-  long long local = tile - __ldg(&P.tile_begin);
-  int tn_ = __ldg(&P.tiles_n);
-  int per = __ldg(&P.tiles_m) * tn_;
+  const unsigned local = (unsigned)(tile - __ldg(&P.tile_begin));      // tiles of one problem < 2^32 (checked by the plan)
+  const unsigned tn_ = (unsigned)__ldg(&P.tiles_n);
+  const unsigned per = (unsigned)__ldg(&P.tiles_m) * tn_;
   TileInfo t;
   t.prob = lo;
   t.batch = (int)(local / per);
-  int r = (int)(local - (long long)t.batch * per);
-  t.tm = r / tn_;
-  t.tn = r - t.tm * tn_;
+  const unsigned r = local - (unsigned)t.batch * per;
+  t.tm = (int)(r / tn_);
+  t.tn = (int)(r - (unsigned)t.tm * tn_);
   return t;
 }
 
@@ -159,44 +164,45 @@ __device__ __forceinline__ void consume_k4(double (&acc)[4][4][4], const double2
 template <int MI, int NI>
 __device__ __forceinline__ void consume_slot(double (&acc)[4][4][4], const double2* as, const double2* bs, int nk4,
                                              unsigned mask_n, unsigned mask_y, unsigned mask_b) {
-  consume_k4<MI, NI>(acc, as, bs, mask_n, mask_y, mask_b);
-  if (nk4 > 1) consume_k4<MI, NI>(acc, as + 4 * LDA, bs + 4 * LDB, mask_n, mask_y, mask_b);
+#pragma unroll 1
+  for (int kk = 0; kk < nk4; ++kk) consume_k4<MI, NI>(acc, as + kk * 4 * LDA, bs + kk * 4 * LDB, mask_n, mask_y, mask_b);
 }
 
 // registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + 2 fk + c of the tile.
-// One instance for all variants (bounds are run-time, accumulator indices compile-time): keeps the code small.
-__device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const TileRec& t, double2* C, int warp, int fr, int fk) {
-  const int mrows = t.mrows, ncols = t.ncols, m0 = t.m0, n0 = t.n0;
-  const gwsig_idx2 cm = t.cm, cn = t.cn;
+// One instance for all variants (bounds are run-time, accumulator indices compile-time).  Lane L computes the offset of
+// tile column L and of the warp's L-th row once; the lanes then fetch the ones they need by shuffle (one idx2 site each).
+__device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const TileRec& t, double2* C, int warp, int lane) {
+  const int fr = lane >> 2, fk = lane & 3;
+  const int mrows = t.mrows, ncols = t.ncols;
   double2* cbase = C + t.c_off;
   const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
-  long long cn_off[4][2];
+  const long long my_col = lane < ncols ? idx2(t.cn, t.n0 + lane) : -1;
+  const int my_row_l = warp * 8 + 32 * (lane >> 3) + (lane & 7);
+  const long long my_row = my_row_l < mrows ? idx2(t.cm, t.m0 + my_row_l) : -1;
+  long long coff[4][2], roff[4];
 #pragma unroll
   for (int j = 0; j < 4; ++j)
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int nl = j * 8 + fk * 2 + c;
-      cn_off[j][c] = nl < ncols ? idx2(cn, n0 + nl) : -1;
-    }
+    for (int c = 0; c < 2; ++c) coff[j][c] = __shfl_sync(0xffffffffu, my_col, j * 8 + fk * 2 + c);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) roff[i] = __shfl_sync(0xffffffffu, my_row, i * 8 + fr);
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    const int ml = (warp + 4 * i) * 8 + fr;
-    if (ml < mrows) {
-      double2* crow = cbase + idx2(cm, m0 + ml);
+    if (roff[i] < 0) continue;
+    double2* crow = cbase + roff[i];
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
+    for (int j = 0; j < 4; ++j)
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
-          if (cn_off[j][c] >= 0) {
-            double2* dst = crow + cn_off[j][c];
-            if (accum) {
-              red_add(&dst->x, acc[i][j][c]);
-              red_add(&dst->y, acc[i][j][2 + c]);
-            } else {
-              *dst = make_double2(acc[i][j][c], acc[i][j][2 + c]);
-            }
+      for (int c = 0; c < 2; ++c)
+        if (coff[j][c] >= 0) {
+          double2* dst = crow + coff[j][c];
+          if (accum) {
+            red_add(&dst->x, acc[i][j][c]);
+            red_add(&dst->y, acc[i][j][2 + c]);
+          } else {
+            *dst = make_double2(acc[i][j][c], acc[i][j][2 + c]);
           }
-    }
+        }
   }
 }
 
@@ -267,12 +273,60 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
         const double2* abase = p.A + __ldg(&S.a_off) + a_boff;
         const bool b_ok = lane < ncols;
         const double2* b_col = p.B + __ldg(&S.b_off) + b_boff + (b_ok ? idx2(S.bn, n0 + lane) : 0);
-        auto publish = [&](int k0) {                      // leader: slot header, then a releasing arrive
-          if (leader) {
+        // A row offsets of this lane (32-bit: element offsets inside a tile stay < 2^31, checked by the plan).
+        //   A contiguous along m: lane <-> tile rows lane + 32 r (r < 4); this warp stages k-rows 2 pw, 2 pw + 1
+        //   A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j, j < 8)
+        const gwsig_idx2 am = S.am;
+        const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
+        int a_roff[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int ml = kmajor ? mr + 16 * j : lane + 32 * j;
+          a_roff[j] = ((kmajor || j < 4) && ml < mrows) ? (int)idx2(am, m0 + ml) : -1;
+        }
+        for (int k0 = 0; k0 < K; k0 += BK) {
+          mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
+          const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
+          const bool two = k0 + 4 < K;                      // the slot's second k4 step holds data
+          if (!kmajor) {
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const int kk = 2 * pw + h2;
+              const int k = k0 + kk;
+              if (kk < 4 || two) {
+                const bool kok = k < K;
+                const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+                  if (a_roff[r] >= 0) cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, kok ? ap + a_roff[r] : abase, kok);
+              }
+            }
+          } else if (kl < 4 || two) {
+            const int k = k0 + kl;
+            const bool kok = k < K;
+            const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              if (a_roff[j] >= 0) cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, kok ? ap + a_roff[j] : abase, kok);
+          }
+          if (b_ok) {
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const int kk = 2 * pw + h2;
+              const int k = k0 + kk;
+              if (kk < 4 || two) {
+                const bool kok = k < K;
+                cp_async16(bs + (unsigned)(kk * LDB + lane) * 16u, b_col + (kok ? idx2(bk, k) : 0), kok);
+              }
+            }
+          }
+          mbar_arrive_cp_async(full0 + 8 * stage);
+          if (leader) {                                     // slot header, then a releasing arrive
             SlotHdr& h = hdr[stage];
             const bool last = last_seg && k0 + BK >= K;
             h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
-            h.nk4 = (K - k0 > 4) ? 2 : 1;
+            h.nk4 = two ? 2 : 1;
             if (first) {
               TileRec& t = trec[tslot];
               t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
@@ -283,78 +337,7 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
             mbar_arrive(full0 + 8 * stage);
           }
           if (first) { first = false; if (++tslot == kStages + 1) tslot = 0; }
-        };
-        // B rows of this warp: kk = 2 pw, 2 pw + 1 (both A layouts); k-rows beyond the slot's last k4 step are not read
-        auto stage_b = [&](int k0, unsigned bs) {
-          if (b_ok) {
-#pragma unroll
-            for (int h2 = 0; h2 < 2; ++h2) {
-              const int kk = 2 * pw + h2;
-              const int k = k0 + kk;
-              if (kk < 4 || k0 + 4 < K) {
-                const bool kok = k < K;
-                cp_async16(bs + (unsigned)(kk * LDB + lane) * 16u, b_col + (kok ? idx2(bk, k) : 0), kok);
-              }
-            }
-          }
-        };
-        if (!kmajor) {
-          // ---- A contiguous along m: lane <-> rows lane + 32 r of the tile; this warp stages k-rows 2 pw, 2 pw + 1 ----
-          const gwsig_idx2 am = S.am;
-          const double2* a_row[4];
-#pragma unroll
-          for (int r = 0; r < 4; ++r) {
-            const int ml = lane + 32 * r;
-            a_row[r] = ml < mrows ? abase + idx2(am, m0 + ml) : nullptr;
-          }
-          for (int k0 = 0; k0 < K; k0 += BK) {
-            mbar_wait(empty0 + 8 * stage, phase ^ 1);
-            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
-            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
-#pragma unroll
-            for (int h2 = 0; h2 < 2; ++h2) {
-              const int kk = 2 * pw + h2;
-              const int k = k0 + kk;
-              if (kk < 4 || k0 + 4 < K) {
-                const bool kok = k < K;
-                const long long ka = kok ? idx2(ak, k) : 0;
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                  if (a_row[r]) cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, a_row[r] + ka, kok);
-              }
-            }
-            stage_b(k0, bs);
-            mbar_arrive_cp_async(full0 + 8 * stage);
-            publish(k0);
-            if (++stage == kStages) { stage = 0; phase ^= 1; }
-          }
-        } else {
-          // ---- A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j) ----
-          const gwsig_idx2 am = S.am;
-          const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
-          int a_roff[8];                                // element offsets inside a tile stay < 2^31 (checked by the plan)
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const int ml = mr + 16 * j;
-            a_roff[j] = ml < mrows ? (int)idx2(am, m0 + ml) : -1;
-          }
-          for (int k0 = 0; k0 < K; k0 += BK) {
-            mbar_wait(empty0 + 8 * stage, phase ^ 1);
-            const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
-            const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
-            if (kl < 4 || k0 + 4 < K) {
-              const int k = k0 + kl;
-              const bool kok = k < K;
-              const double2* ap = abase + (kok ? idx2(ak, k) : 0);
-#pragma unroll
-              for (int j = 0; j < 8; ++j)
-                if (a_roff[j] >= 0) cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, kok ? ap + a_roff[j] : abase, kok);
-            }
-            stage_b(k0, bs);
-            mbar_arrive_cp_async(full0 + 8 * stage);
-            publish(k0);
-            if (++stage == kStages) { stage = 0; phase ^= 1; }
-          }
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
     }
@@ -406,7 +389,7 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
       // ---- epilogue after the last slot of a tile ----------
       if ((ctl & 2) && variant >= 0) {
         const TileRec& t = trec[tslot];
-        store_tile(acc, t, p.C, warp, fr, fk);
+        store_tile(acc, t, p.C, warp, lane);
       }
     }
   }

@@ -26,7 +26,7 @@ ZG_HD int zg_tiles_m(int M) { return (M + ZG_BM - 1) / ZG_BM; }
 ZG_HD int zg_tiles_n(int N) { return ((N + 7) / 8 + ZG_NG_MAX - 1) / ZG_NG_MAX; }
 ZG_HD void zg_ntile(int N, int tiles_n, int tn, int& n0, int& ncols) {
   const int G = (N + 7) / 8;
-  const int g0 = (int)(((long long)tn * G) / tiles_n), g1 = (int)(((long long)(tn + 1) * G) / tiles_n);
+  const int g0 = (tn * G) / tiles_n, g1 = ((tn + 1) * G) / tiles_n;      // G < 2^27 / tiles_n: no overflow
   n0 = 8 * g0;
   const int n1 = 8 * g1 < N ? 8 * g1 : N;
   ncols = n1 - n0;
