@@ -373,7 +373,12 @@ def main():
             for w, bps in ((4, 2), (8, 2), (8, 4), (16, 2), (16, 4)):
                 best = max(best, lib.probe_fp64(kind, w, bps, 20000)[0])
             out[nm] = best
-        print(json.dumps({"fp64_probe_tflops": out}))
+        tf1, ms1 = lib.probe_fp64(3, 4, 1, 20000)        # one chain per warp, one warp per SM sub-partition
+        n_dmma = 20000 * 16
+        sm_hz = 1.965e9
+        lat = {"dependent_dmma_cycles_at_1965MHz": ms1 * 1e-3 * sm_hz / n_dmma, "ms": ms1, "chain_length": n_dmma}
+        print(json.dumps({"fp64_probe_tflops": out, "dmma_issue_cycles_per_subpartition": 512.0 * 148 * 4 * sm_hz / (out["dmma"] * 1e12),
+                          "dmma_latency": lat}))
         return
 
     mode = MODES[args.mode]

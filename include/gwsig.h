@@ -182,7 +182,8 @@ int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, vo
 
 /* ---- FP64 peak probe (measurement support; needs a device) -------------------------------------
  * kind 0: register-only mma.sync.m8n8k4.f64 issue-rate loop; kind 1: register-only DFMA loop;
- * kind 2: both interleaved in every warp (tells whether DMMA and DFMA share one pipe).
+ * kind 2: both interleaved in every warp (tells whether DMMA and DFMA share one pipe); kind 3: one
+ * dependent DMMA chain per warp (with 4 warps per block and 1 block per SM: the DMMA latency).
  * Returns achieved TFLOP/s over `iters` inner iterations on every SM (CUDA-event timed).           */
 int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters,
                      double* tflops, double* ms);

@@ -691,7 +691,7 @@ int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, co
 
 int gwsig_probe_fp64(gwsig_ctx* ctx, int kind, int warps_per_block, int blocks_per_sm, int64_t iters, double* tflops,
                      double* ms) {
-  if (!ctx || !tflops || kind < 0 || kind > 2 || warps_per_block < 1 || warps_per_block > 32 || blocks_per_sm < 1 || iters < 1) return GWSIG_ERR_ARG;
+  if (!ctx || !tflops || kind < 0 || kind > 3 || warps_per_block < 1 || warps_per_block > 32 || blocks_per_sm < 1 || iters < 1) return GWSIG_ERR_ARG;
   int rc = ensure_cuda(ctx);
   if (rc) return rc;
   CU(cudaSetDevice(ctx->device));

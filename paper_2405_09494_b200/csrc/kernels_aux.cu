@@ -151,6 +151,9 @@ cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long it
   } else if (kind == 1) {
     probe_dfma_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
     *flops_out = (double)blocks * warps_per_block * 32.0 * (double)iters * NACC * 2.0;
+  } else if (kind == 3) {      // ONE dependent chain per warp: with 1 warp per sub-partition this is the DMMA latency
+    probe_dmma_kernel<1><<<blocks, warps_per_block * 32, 0, stream>>>(iters * NACC, sink);
+    *flops_out = (double)blocks * warps_per_block * (double)iters * NACC * 512.0;
   } else {
     probe_mixed_kernel<NACC><<<blocks, warps_per_block * 32, 0, stream>>>(iters, sink);
     *flops_out = (double)blocks * warps_per_block * (double)iters * NACC * (512.0 + 8 * 32 * 2.0);
