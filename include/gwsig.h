@@ -107,6 +107,14 @@ int gwsig_set_symmetry(gwsig_ctx* ctx, int nops, const int* rot, const double* t
 int gwsig_set_blocks(gwsig_ctx* ctx, const int* nblk_ao, const int* ao_block_off, const int* nblk_aux,
                      const int* aux_block_off, const double* U_ao, const double* U_aux);
 
+/* set_output_points (host, optional, after set_symmetry and before set_triples): evaluate Sigma only at
+ * the n listed k1 (wedge representatives in the IBZ modes, any mesh point in FULL_BZ) instead of at all of
+ * them.  "One representative is chosen" per star and every output k1 is an independent sum
+ * over q (Eq. 16), so this is also how the work would be dealt to several GPUs (the paper distributes
+ * (k1,k2) pairs).  Pairs become q * n + i1 over the listed points; inputs G, W keep their
+ * layout; V2 and Sigma carry the listed points only.  Errors: GWSIG_ERR_ARG (not a wedge point, repeated). */
+int gwsig_set_output_points(gwsig_ctx* ctx, int n, const int* k_list);
+
 /* set_triples (IBZ_BLOCK only, host): symmetry-allowed blocks of V2 for every pair ("only non-zero
  * blocks are considered").  triple_ptr[npairs+1] CSR; triples[3*nt] = (p, alpha, iota):
  * aux block of q, orbital block of k2, orbital block of k1; sorted by p within a pair.              */

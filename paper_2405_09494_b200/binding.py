@@ -34,14 +34,15 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_set_symmetry", "gwsig_set_blocks", "gwsig_set_triples", "gwsig_get_ibz", "gwsig_pair_count",
            "gwsig_pair_info", "gwsig_buffer_sizes", "gwsig_sigma_begin", "gwsig_sigma_push_pairs", "gwsig_sigma_end",
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
-           "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host"]
+           "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host",
+           "gwsig_set_output_points"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
     "gwsig_create": [C.POINTER(_vp), _i], "gwsig_destroy": [_vp],
     "gwsig_set_lattice": [_vp, _vp, _vp, _i, _i, _i, _d], "gwsig_set_atoms": [_vp, _i, _vp, _vp, _vp],
     "gwsig_set_symmetry": [_vp, _i, _vp, _vp, _vp, _vp, _vp, _i], "gwsig_set_blocks": [_vp, _vp, _vp, _vp, _vp, _vp, _vp],
-    "gwsig_set_triples": [_vp, _i64, _vp, _vp], "gwsig_get_ibz": [_vp, _vp, _vp, _vp, _vp],
+    "gwsig_set_triples": [_vp, _i64, _vp, _vp], "gwsig_set_output_points": [_vp, _i, _vp], "gwsig_get_ibz": [_vp, _vp, _vp, _vp, _vp],
     "gwsig_pair_count": [_vp, _vp, _vp], "gwsig_pair_info": [_vp, _i64, _vp, _vp, _vp, _vp, _vp],
     "gwsig_buffer_sizes": [_vp, _vp, _vp, _vp, _vp], "gwsig_sigma_begin": [_vp, _vp, _vp, _vp, _vp],
     "gwsig_sigma_push_pairs": [_vp, _i64, _i64, _vp], "gwsig_sigma_end": [_vp],
@@ -132,6 +133,10 @@ class Gwsig:
         ux = None if U_aux is None else _np(U_aux, np.complex128)
         self._ck(_lib.gwsig_set_blocks(self._h, nb_ao.ctypes.data, cat_ao.ctypes.data, nb_ax.ctypes.data, cat_ax.ctypes.data,
                                        _ptr(ua), _ptr(ux)))
+
+    def set_output_points(self, k_list):
+        k = _np(k_list, np.int32)
+        self._ck(_lib.gwsig_set_output_points(self._h, len(k), _ptr(k)))
 
     def set_triples(self, triple_ptr, triples):
         tp = _np(triple_ptr, np.int64)

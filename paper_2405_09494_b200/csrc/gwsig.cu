@@ -358,6 +358,13 @@ int gwsig_set_blocks(gwsig_ctx* ctx, const int* nblk_ao, const int* ao_block_off
   return rc ? fail(ctx, rc, ctx->plan.err) : rc;
 }
 
+int gwsig_set_output_points(gwsig_ctx* ctx, int n, const int* k_list) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  invalidate(ctx);
+  int rc = ctx->plan.set_output_points(n, k_list);
+  return rc ? fail(ctx, rc, ctx->plan.err) : rc;
+}
+
 int gwsig_set_triples(gwsig_ctx* ctx, int64_t npairs, const int64_t* triple_ptr, const int32_t* triples) {
   if (!ctx) return GWSIG_ERR_ARG;
   invalidate(ctx);

@@ -168,6 +168,24 @@ int Plan::set_symmetry(int nops_, const int* rot_, const double* trans_, const d
   return finalize_layouts();
 }
 
+int Plan::set_output_points(int n, const int* k_list) {
+  if (!have_sym) { err = "set_output_points: call set_symmetry first"; return GWSIG_ERR_ARG; }
+  if (n < 1 || n > nk || !k_list) { err = "set_output_points: bad count or NULL list"; return GWSIG_ERR_ARG; }
+  std::vector<char> seen(nk, 0);
+  for (int i = 0; i < n; ++i) {
+    const int k = k_list[i];
+    if (k < 0 || k >= nk || seen[k]) { err = "set_output_points: point out of range or repeated"; return GWSIG_ERR_ARG; }
+    if (mode != GWSIG_FULL_BZ && ir_index[k] < 0) { err = "set_output_points: point " + std::to_string(k) + " is not a wedge representative"; return GWSIG_ERR_ARG; }
+    seen[k] = 1;
+  }
+  out_list.assign(k_list, k_list + n);
+  nk1 = n;
+  npairs = (long long)nk * nk1;
+  have_triples = false;
+  triple_ptr.clear(); triples.clear();
+  return finalize_layouts();
+}
+
 int Plan::set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nblk_aux, const int* aux_block_off,
                      const double* U_ao_, const double* U_aux_) {
   if (!have_sym || mode != GWSIG_IBZ_BLOCK) { err = "set_blocks: needs set_symmetry with GWSIG_IBZ_BLOCK"; return GWSIG_ERR_ARG; }
@@ -231,7 +249,9 @@ int Plan::set_triples(int64_t npairs_, const int64_t* triple_ptr_, const int32_t
 int Plan::finalize_layouts() {
   const bool blk = mode == GWSIG_IBZ_BLOCK;
   // input G / W: per wedge point (IBZ modes) or per mesh point (FULL_BZ), packed blocks in block mode
-  const std::vector<int>& pts = mode == GWSIG_FULL_BZ ? out_list : ir_list;
+  std::vector<int> all_k(nk);
+  std::iota(all_k.begin(), all_k.end(), 0);
+  const std::vector<int>& pts = mode == GWSIG_FULL_BZ ? all_k : ir_list;     // inputs do not depend on the output points
   g_in_off.assign(pts.size() + 1, 0);
   w_in_off.assign(pts.size() + 1, 0);
   for (size_t i = 0; i < pts.size(); ++i) {

@@ -69,6 +69,7 @@ struct Plan {
                    const int* shift_, int mode_);
   int set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nblk_aux, const int* aux_block_off,
                  const double* U_ao_, const double* U_aux_);
+  int set_output_points(int n, const int* k_list);
   int set_triples(int64_t npairs_, const int64_t* triple_ptr_, const int32_t* triples_);
   int finalize_layouts();
 

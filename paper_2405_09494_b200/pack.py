@@ -15,7 +15,7 @@ class Configured:
     """a Gwsig context with lattice / symmetry (/ blocks) set, plus the host pre-step objects."""
 
     def __init__(self, lib: Gwsig, mode: int, a, mesh, nao, naux, ntau, beta, pos, ao_atom, aux_atom,
-                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7):
+                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7, out_points=None):
         self.lib, self.mode = lib, mode
         self.nao, self.naux, self.ntau = nao, naux, ntau
         lib.set_lattice(a, mesh, nao, naux, ntau, beta)
@@ -30,9 +30,13 @@ class Configured:
             lib.set_symmetry(W, w, P_ao, P_aux, shift, mode)
             self.setup = SymSetup(mesh, W, w, shift, P_ao, P_aux, ao_atom, aux_atom, seed=seed)
         self.ir_list, self.ir_of, self.op_of = lib.get_ibz()
+        if callable(out_points):                       # e.g. lambda wedge: wedge[:2]
+            out_points = out_points(np.arange(lib.nk) if mode == FULL_BZ else self.ir_list)
+        if out_points is not None:
+            lib.set_output_points(out_points)
         self.npairs, self.nk1 = lib.pair_count()
         self.nk = lib.nk
-        self.out_list = np.arange(self.nk) if mode == FULL_BZ else self.ir_list
+        self.out_list = (np.arange(self.nk) if mode == FULL_BZ else self.ir_list) if out_points is None else np.asarray(out_points)
         if mode == IBZ_BLOCK:
             self.ao, self.aux = self.setup.adapt("ao"), self.setup.adapt("aux")
             lib.set_blocks(self.ao.off, self.aux.off)
@@ -41,7 +45,7 @@ class Configured:
     def pack_GW(self, G_of, W_of):
         """G_of(k) -> [ntau,nao,nao], W_of(q) -> [ntau,naux,naux] in the orbital basis.
         Returns flat complex128 arrays in the layout of the current mode."""
-        pts = self.out_list if self.mode == FULL_BZ else self.ir_list
+        pts = np.arange(self.nk) if self.mode == FULL_BZ else self.ir_list
         if self.mode != IBZ_BLOCK:
             G = np.stack([G_of(int(k)) for k in pts]).ravel()
             W = np.stack([W_of(int(k)) for k in pts]).ravel()
@@ -97,8 +101,8 @@ class Configured:
         return out
 
 
-def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7) -> Configured:
+def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7, out_points=None) -> Configured:
     """convenience for the synthetic crystals of gwsig_synth (any object with the same fields)."""
     sg = cr.sg
     return Configured(lib, mode, cr.a, cr.mesh, cr.nao, cr.naux, cr.ntau, cr.beta, cr.pos, cr.ao_atom, cr.aux_atom,
-                      W=sg.W, w=sg.w, shift=sg.shift, P_ao=cr.P_ao, P_aux=cr.P_aux, seed=seed)
+                      W=sg.W, w=sg.w, shift=sg.shift, P_ao=cr.P_ao, P_aux=cr.P_aux, seed=seed, out_points=out_points)

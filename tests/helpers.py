@@ -40,7 +40,7 @@ def fold_to_orbital(cfg, inp, sigma_list):
         return out
     cr = inp.cr
     for k in range(cfg.nk):
-        if k in out:
+        if k in out or int(cfg.ir_of[k]) not in out:     # (a restricted set of output points leaves stars out)
             continue
         g = int(cfg.op_of[k])
         O = rep_at_k(cr.P_ao[g], cr.ao_atom, cr.sg.shift[g], cr.kmesh.frac[k])

@@ -125,6 +125,47 @@ def _setup_full_from_crystal(name):
     return B, inp, cfg, G, W, V
 
 
+def _sampled(name, mode, pick, taus, pushes_q=None):
+    """BASELINE configs too large for a full oracle run: Sigma at a few wedge points (every output k1 is an
+    independent sum over all q, gwsig_set_output_points), all tau on the GPU, oracle at the sampled tau."""
+    B = _B()
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    inp = make_inputs(name)
+    lib = B.Gwsig(device=0)
+    cfg = configure_from_crystal(lib, inp.cr, mode, out_points=pick)
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    V = cfg.pack_V(inp.V2_rows)
+    sig = run_gpu(cfg, G, W, V, pushes=None if pushes_q is None else pushes_q * cfg.nk1)
+    w = _check(cfg, inp, sig, ks=[int(k) for k in cfg.out_list], taus=taus)
+    print(name, "mode", mode, "points", list(cfg.out_list), "tau", list(taus), "worst rel err", w)
+
+
+def test_output_point_subset_matches_full_run():
+    B, inp, cfg, G, W, V = _setup("toy_diamond", 2)
+    full = cfg.unpack_sigma(run_gpu(cfg, G, W, V))
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    lib2 = B.Gwsig(device=0)
+    cfg2 = configure_from_crystal(lib2, inp.cr, 2, out_points=lambda wedge: [wedge[2], wedge[0]])
+    G2, W2 = cfg2.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    sub = cfg2.unpack_sigma(run_gpu(cfg2, G2, W2, cfg2.pack_V(inp.V2_rows)))
+    for a, i in enumerate((2, 0)):
+        assert np.abs(sub[a] - full[i]).max() <= 1e-13 * np.abs(full[i]).max()
+
+
+def test_cfg3_sampled():
+    _sampled("cfg3", 2, lambda wedge: [wedge[0], wedge[5], wedge[-1]], [0, 51, 103])
+    _sampled("cfg3", 1, lambda wedge: [wedge[3]], [7], pushes_q=54)
+
+
+def test_cfg4_sampled():
+    _sampled("cfg4", 2, lambda wedge: [wedge[0], wedge[9]], [0, 127])
+    _sampled("cfg4", 1, lambda wedge: [wedge[-1]], [64], pushes_q=24)
+
+
+def test_cfg5_sampled():
+    _sampled("cfg5", 2, lambda wedge: [wedge[0], wedge[-1]], [0, 135])
+
+
 def test_hermitize_option_and_observed_hermiticity():
     B, inp, cfg, G, W, V = _setup("toy_diamond", 1)
     s0 = run_gpu(cfg, G, W, V)

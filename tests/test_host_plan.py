@@ -122,3 +122,46 @@ def test_descriptors_reproduce_oracle(name, mode, push, nt):
     if mode == B.IBZ_BLOCK:
         full, ex = lib.flop_counts()
         assert 0 < ex < full * len(cfg.ir_list) / inp.nk
+
+
+def test_output_points_subset_descriptors():
+    """gwsig_set_output_points: Sigma at a listed subset of wedge points equals the same rows of the full plan."""
+    inp = make_inputs("toy_diamond")
+    cfgs = []
+    for pick in (None, lambda wedge: [wedge[1]]):
+        lib = B.Gwsig(device=-1)
+        cfg = configure_from_crystal(lib, inp.cr, B.IBZ_BLOCK, out_points=pick)
+        G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+        V = cfg.pack_V(inp.V2_rows)
+        cfgs.append((cfg, cfg.unpack_sigma(run_plan_numpy(cfg, inp, G, W, V))))
+    (full_cfg, full), (sub_cfg, sub) = cfgs
+    assert sub_cfg.npairs == inp.nk and list(sub_cfg.out_list) == [full_cfg.ir_list[1]]
+    assert np.abs(sub[0] - full[1]).max() <= 1e-13 * np.abs(full[1]).max()
+    lib = B.Gwsig(device=-1)
+    with pytest.raises(B.GwsigError) as e:             # not a wedge representative
+        non_wedge = [k for k in range(inp.nk) if k not in set(full_cfg.ir_list)][0]
+        configure_from_crystal(lib, inp.cr, B.IBZ, out_points=[non_wedge])
+    assert e.value.code == -1
+
+
+def test_stage3_split_k_parts_tile_the_segments():
+    """stage 3 cuts long segment lists into parts (and segments along P') that add into one Sigma block: the parts of
+    a block must cover every (pair, triple, P') exactly once -- checked through the interpreter on a config whose K is
+    long enough to be cut (ntau small keeps it cheap)."""
+    inp = make_inputs("toy_diamond4")
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ, out_points=lambda wedge: [wedge[0], wedge[3]])
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    V = cfg.pack_V(inp.V2_rows)
+    pr, sg, _ = lib.plan_get(0, cfg.npairs, 1, 3)
+    ksum = {}
+    for P in pr:
+        ksum[int(P["c_off"])] = ksum.get(int(P["c_off"]), 0) + sum(int(sg[s]["K"]) for s in range(P["seg_begin"], P["seg_begin"] + P["seg_count"]))
+    assert len(pr) > len(ksum), "expected split-K parts"          # more problems than output blocks
+    assert all(v == inp.nk * inp.naux * inp.nao for v in ksum.values())
+    sig = run_plan_numpy(cfg, inp, G, W, V)
+    got = cfg.unpack_sigma(sig)
+    ref = oracle_sigma(inp, [int(k) for k in cfg.out_list])
+    for a in range(len(cfg.out_list)):
+        for t in range(inp.ntau):
+            assert rel_err(got[a][t], ref[a, t]) < 1e-12
