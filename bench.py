@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-sample-tau", type=int, default=4, help="tau points of the oracle sample")
+    ap.add_argument("--engine", type=int, default=0, choices=[0, 2], help="0: DMMA 3M kernel (default), 2: DMMA 4M kernel")
     ap.add_argument("--probe-only", action="store_true", help="print the FP64 issue-rate probes and exit")
     return ap.parse_args()
 
@@ -313,10 +314,7 @@ def reference_main(args, rank, world):
     if args.workload == "cfg1":
         ir = list(range(inp.nk))
     else:
-        from paper_2405_09494_b200 import build as gw_build
-        gw_build.build()
-        from paper_2405_09494_b200 import binding as B, pack
-        ir = list(pack.configure_from_crystal(B.Gwsig(device=-1), inp.cr, B.IBZ).ir_list)
+        ir = [int(k) for k in inp.kmesh.stars(inp.cr.sg)[0]]       # the generator's own star finder: no product code in this arm
     ks, taus = sample_points(ir, inp.ntau, 1, args.cpu_sample_tau)
     for _ in range(max(args.warmup, 0)):
         oracle_sample(inp, ks[:1], taus[:1])
@@ -387,6 +385,7 @@ def main():
     t_setup = time.time()
     wl = Workload(args.workload, mode, B, pack, torch=torch, dev=dev, device_index=local)
     cfg, lib = wl.cfg, wl.lib
+    lib.set_option("engine", args.engine)
     t_setup = time.time() - t_setup
 
     # ---- the timed region: W warm-up steps, then exactly K steps between barrier + synchronize --------------
@@ -420,7 +419,7 @@ def main():
     line = {"metric": METRIC, "value": ms_eval, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex128 (f64)", "data": "synthetic",
-            "config": {"workload": f"{args.workload} ({describe(args.workload)})", "mode": args.mode, "nk": int(cfg.nk), "nik": int(cfg.nk1),
+            "config": {"workload": f"{args.workload} ({describe(args.workload)})", "mode": args.mode, "engine": {0: "dmma 3M", 2: "dmma 4M"}[args.engine], "nk": int(cfg.nk), "nik": int(cfg.nk1),
                        "nao": int(cfg.nao), "naux": int(cfg.naux), "ntau": int(cfg.ntau), "pairs": int(cfg.npairs),
                        "l2": "inputs larger than L2 (V alone is %.2f GB)" % (wl.V.numel() * 16 / 1e9 if torch.is_tensor(wl.V) else wl.V.nbytes / 1e9),
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": round(t_setup, 1)},
@@ -444,14 +443,14 @@ def main():
                            "stage_gflop": [x / 1e9 for x in sf]}
     dom = int(np.argmax([t1, t2, t3]))
     ach = sf[dom] / max((t1, t2, t3)[dom], 1e-12) / 1e12
-    line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + " (zgemm_grouped_dmma)",
+    line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + (" (zgemm_grouped_dmma3m)" if args.engine == 0 else " (zgemm_grouped_dmma)"),
                         "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
                         "peak_source": "FP64 tensor (DMMA) peak derived from unit counts x max clock, 148 x 128 flop/clk x 1.965 GHz; "
                                        "the register-only DMMA probe of this library reaches 36.9 (MEASURED_PEAKS.json has no FP64 entry)"}
 
     # ---- end to end through the host-buffer call ------------------------------------------------------------------
     if not args.no_e2e:
-        et, h2d, d2h, hs = run_e2e(wl, torch, dev, max(1, min(args.steps, 2)), 1)
+        et, h2d, d2h, hs = run_e2e(wl, torch, dev, args.steps, max(1, min(args.warmup, 2)))
         line["e2e"] = {"value": float(np.mean(et)) * 1e3, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                        "api": "gwsig_sigma_eval_host (pinned host G, W, V -> host Sigma; V streamed through a 2-slot ring)"}
         assert np.abs(hs - sigma_gpu).max() <= 1e-12 * np.abs(sigma_gpu).max(), "host-buffer path disagrees with the resident path"

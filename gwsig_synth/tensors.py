@@ -12,6 +12,8 @@ Recipe (stated again in DESIGN.md):
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 
 from .crystal import Crystal
@@ -134,13 +136,19 @@ def _encode(R: np.ndarray) -> np.ndarray:
     return key
 
 
-def _group_average(cr: Crystal, keys: np.ndarray, M: np.ndarray, transform, starts, nleg: int):
+def _group_average(cr: Crystal, keys: np.ndarray, M: np.ndarray, reps, starts, nleg: int):
     """Shared bookkeeping of the group average (G7/G8).  ``keys`` [n, 3*(nleg-1)]
     are the lattice vectors R (two-index) or (R1, R2) (three-index) of the
     stacked real-space blocks ``M`` [n, ...]; leg 0 sits in cell 0, leg j>0 in
     cell R_j.  Under g an atom block (x_0, .., x_m) at (R_1, ..) moves to
-    (perm x_0, .., perm x_m) at (W R_j + s_{x_j} - s_{x_0}); ``transform(g, M)``
-    applies the real representation matrices to all legs."""
+    (perm x_0, .., perm x_m) at (W R_j + s_{x_j} - s_{x_0}) and every leg j is
+    multiplied by the real representation matrix ``reps[j][g]`` (perm (x) Wigner D).
+    The representation matrices only connect atom x to perm x, so each atom block
+    is transformed on its own with the matching sub-matrices (same result as
+    transforming the whole tensor, a fraction of the work); operations run on a
+    small thread pool, the accumulation into the output is serialised."""
+    import threading
+    from concurrent.futures import ThreadPoolExecutor
     sg = cr.sg
     nat = cr.natom
     nR = nleg - 1
@@ -154,19 +162,38 @@ def _group_average(cr: Crystal, keys: np.ndarray, M: np.ndarray, transform, star
 
     allk = np.concatenate([new_keys(g, c) for g in range(sg.nops) for c in combos])
     uniq = np.unique(_encode(allk))
+    del allk
     out = np.zeros((len(uniq),) + M.shape[1:])
     out_keys = np.zeros((len(uniq), 3 * nR), dtype=np.int64)
-    for g in range(sg.nops):
-        T = transform(g, M)
+    lock = threading.Lock()
+
+    def one_op(g):
         perm = sg.perm[g]
         for c in combos:
+            sin = tuple(slice(starts[j][c[j]], starts[j][c[j] + 1]) for j in range(nleg))
+            sout = tuple(slice(starts[j][perm[c[j]]], starts[j][perm[c[j]] + 1]) for j in range(nleg))
+            B = np.ascontiguousarray(M[(slice(None),) + sin])
+            for j in range(nleg):                                   # leg j: D[out rows, in cols] on axis 1 + j
+                D = np.ascontiguousarray(reps[j][g][sout[j], sin[j]])
+                if j == nleg - 1:
+                    B = (B.reshape(-1, B.shape[-1]) @ D.T).reshape(B.shape)
+                elif j == 0:
+                    B = np.matmul(D, B.reshape(B.shape[0], B.shape[1], -1)).reshape(B.shape)
+                else:
+                    B = np.matmul(D[None, None], B)
             nk_ = new_keys(g, c)
             idx = np.searchsorted(uniq, _encode(nk_))
-            out_keys[idx] = nk_
-            sl = tuple(slice(starts[j][perm[c[j]]], starts[j][perm[c[j]] + 1]) for j in range(nleg))
-            out[(idx,) + sl] += T[(slice(None),) + sl]
+            with lock:
+                out_keys[idx] = nk_
+                out[(idx,) + sout] += B
+
+    nthreads = max(1, min(4, (os.cpu_count() or 1) // 2))
+    with ThreadPoolExecutor(nthreads) as pool:
+        list(pool.map(one_op, range(sg.nops)))
     out /= sg.nops
     keep = np.abs(out).reshape(len(uniq), -1).max(axis=1) > 0
+    if keep.all():
+        return out_keys, out
     return out_keys[keep], out[keep]
 
 
@@ -175,7 +202,7 @@ def average_two_index(cr: Crystal, Xr: dict, P: np.ndarray, start: np.ndarray) -
     (g.X)_{(pi(x) i'),(pi(y) j')}(W R + s_y - s_x) += D_{i'i} D_{j'j} X_{(x i),(y j)}(R)   (G7)."""
     keys = np.array(list(Xr.keys()), dtype=np.int64)
     M = np.stack([Xr[tuple(k)] for k in keys])
-    ok, om = _group_average(cr, keys, M, lambda g, A: P[g] @ A @ P[g].T, (start, start), 2)
+    ok, om = _group_average(cr, keys, M, (P, P), (start, start), 2)
     return {tuple(int(v) for v in k): m for k, m in zip(ok, om)}
 
 
@@ -183,19 +210,17 @@ def average_three_index(cr: Crystal, Vr: dict) -> dict:
     """(1/|G|) sum_g g.V with
     (g.V)_{(pi(z)Q'),(pi(x)i'),(pi(y)j')}(W R1 + s_x - s_z, W R2 + s_y - s_z)
         += Daux_{Q'Q} D_{i'i} D_{j'j} V_{Q,i,j}(R1,R2)                                (G8)."""
-    na, no = cr.naux, cr.nao
     klist = list(Vr.keys())
     keys = np.array([list(k[0]) + list(k[1]) for k in klist], dtype=np.int64)
     M = np.stack([Vr[k] for k in klist])
-
-    def transform(g, A):
-        Pa, Po = cr.P_aux[g], cr.P_ao[g]
-        T = np.matmul(Pa, A.reshape(len(A), na, no * no)).reshape(len(A), na, no, no)
-        T = np.matmul(Po[None, None], T)            # i leg
-        return np.matmul(T, Po.T[None, None])       # j leg
-
-    ok, om = _group_average(cr, keys, M, transform, (cr.aux_start, cr.ao_start, cr.ao_start), 3)
+    ok, om = _group_average(cr, keys, M, (cr.P_aux, cr.P_ao, cr.P_ao), (cr.aux_start, cr.ao_start, cr.ao_start), 3)
     return {(tuple(int(v) for v in k[:3]), tuple(int(v) for v in k[3:])): m for k, m in zip(ok, om)}
+
+
+def _cdot_real(f: np.ndarray, X: np.ndarray, axis: int) -> np.ndarray:
+    """sum_r f[r] X[..r..] over `axis` of the REAL table X with complex weights f, as two real contractions
+    (np.tensordot would first cast the whole table to complex: 30 GB at config 5)."""
+    return np.tensordot(f.real, X, axes=(0, axis)) + 1j * np.tensordot(f.imag, X, axes=(0, axis))
 
 
 class SymmetricInputs:
@@ -276,7 +301,7 @@ class SymmetricInputs:
         """V^{k1,k2}_{Q,ij}  [naux, nao, nao]"""
         f1 = np.exp(-2j * np.pi * (self.vR1 @ self.kmesh.frac[k1]))
         f2 = np.exp(+2j * np.pi * (self.vR2 @ self.kmesh.frac[k2]))
-        T = np.tensordot(f2, self.Vd, axes=(0, 1))                   # [nR1, nel]
+        T = _cdot_real(f2, self.Vd, 1)                               # [nR1, nel]
         return (f1 @ T).reshape(self.naux, self.nao, self.nao)
 
     def V2_rows(self, k1: int, k2s) -> np.ndarray:
@@ -284,7 +309,7 @@ class SymmetricInputs:
         (first momentum k2 carries e^{-2 pi i k2.R1}, second k1 carries e^{+2 pi i k1.R2})."""
         k2s = np.asarray(list(k2s))
         f2 = np.exp(+2j * np.pi * (self.vR2 @ self.kmesh.frac[k1]))
-        T = np.tensordot(f2, self.Vd, axes=(0, 1))                   # [nR1, nel]
+        T = _cdot_real(f2, self.Vd, 1)                               # [nR1, nel]
         f1 = np.exp(-2j * np.pi * (self.kmesh.frac[k2s] @ self.vR1.T))   # [nk2, nR1]
         return (f1 @ T).reshape(len(k2s), self.naux, self.nao, self.nao)
 
@@ -293,7 +318,7 @@ class SymmetricInputs:
         """V^{k1,k2}_{Q,ia} for every k2 in k2s  [len, naux, nao, nao]  (same Bloch sum as V_pair, batched over k2)."""
         k2s = np.asarray(list(k2s))
         f1 = np.exp(-2j * np.pi * (self.vR1 @ self.kmesh.frac[k1]))
-        T = np.tensordot(f1, self.Vd, axes=(0, 0))                   # [nR2, nel]
+        T = _cdot_real(f1, self.Vd, 0)                               # [nR2, nel]
         f2 = np.exp(+2j * np.pi * (self.kmesh.frac[k2s] @ self.vR2.T))   # [nk2, nR2]
         return (f2 @ T).reshape(len(k2s), self.naux, self.nao, self.nao)
 

@@ -47,8 +47,10 @@ typedef enum {
 } gwsig_mode;
 
 typedef enum {
-  GWSIG_ENGINE_DMMA = 0,     /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA)       */
-  GWSIG_ENGINE_REFERENCE = 1 /* one-thread-per-element DFMA kernels on the same plan (debug)      */
+  GWSIG_ENGINE_DMMA = 0,      /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA), complex product by
+                                 the 3M / Karatsuba scheme: 3 real DMMA per complex 8x8x4 block (default)           */
+  GWSIG_ENGINE_REFERENCE = 1, /* one-thread-per-element DFMA kernels on the same plan (debug)                       */
+  GWSIG_ENGINE_DMMA_4M = 2    /* tensor-core kernel with the conventional 4-product complex multiply               */
 } gwsig_engine;
 
 /* kernel kinds for gwsig_kernel_times (steps a1..a6 of DESIGN.md) */

@@ -423,7 +423,7 @@ int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
   if (!ctx || !key) return GWSIG_ERR_ARG;
   std::string k(key);
   if (k == "engine") {
-    if (value != GWSIG_ENGINE_DMMA && value != GWSIG_ENGINE_REFERENCE) return fail(ctx, GWSIG_ERR_ARG, "set_option: bad engine");
+    if (value != GWSIG_ENGINE_DMMA && value != GWSIG_ENGINE_REFERENCE && value != GWSIG_ENGINE_DMMA_4M) return fail(ctx, GWSIG_ERR_ARG, "set_option: bad engine");
     ctx->engine = (int)value;
   } else if (k == "hermitize") ctx->hermitize = value != 0;
   else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
@@ -545,27 +545,8 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
   CU(cudaSetDevice(ctx->device));
   const double2* Vbase = (const double2*)dV;
   const int nk1 = P.nk1;
-  const int q_first = (int)(p0 / nk1), q_last = (int)((p0 + np - 1) / nk1);
 
-  // [a2] unfold W for the q of this push (Eq. 25; Algorithm 4 line 6)
-  const double2* Wsrc = ctx->dW;
-  if (P.mode == GWSIG_IBZ) {
-    const int nq = q_last - q_first + 1;
-    CU(ctx->wring.ensure((size_t)nq * P.ntau * P.naux * P.naux * sizeof(double2)));
-    UnfoldParams up;
-    up.src = ctx->dW; up.dst = (double2*)ctx->wring.p;
-    up.tgt_src = (const int*)ctx->tgt_src.p + q_first; up.tgt_op = (const int*)ctx->tgt_op.p + q_first;
-    up.colphase = (const double2*)ctx->colphase_aux.p + (size_t)q_first * P.naux;
-    up.ell_cols = (const int*)ctx->ell_cols_aux.p; up.ell_vals = (const double*)ctx->ell_vals_aux.p;
-    up.ell_cnt = (const int*)ctx->ell_cnt_aux.p;
-    up.n = P.naux; up.ntau = P.ntau; up.maxnz = ctx->maxnz_aux;
-    int rc = tic(ctx, GWSIG_KIND_UNFOLD_W);
-    if (rc) return rc;
-    CU(launch_unfold_sparse(up, nq, ctx->stream));
-    if ((rc = toc(ctx))) return rc;
-    ctx->launches++;
-    Wsrc = (const double2*)ctx->wring.p;
-  }
+  const double2* Wsrc = P.mode == GWSIG_IBZ ? nullptr : ctx->dW;     // IBZ: the ring, filled per sub-batch below
   const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
 
   // sub-batches of pairs (whole q's where possible) and tau chunks sized to the scratch budget
@@ -589,10 +570,30 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
     CU(ctx->xbuf.ensure(xbytes));
     CU(ctx->ybuf.ensure(xbytes));
     const double2* Vsub = Vbase + (P.v_off[s0] - P.v_off[p0]);
+    const int q_sub = (int)(s0 / nk1);                 // first q of this sub-batch = first q held by the W ring
+    if (P.mode == GWSIG_IBZ) {
+      // [a2] unfold W for the q of this sub-batch only (Eq. 25; Algorithm 4 line 6): the ring holds a few
+      // q, never the whole zone (100 GB at cfg5)
+      const int nq = (int)((s1 - 1) / nk1) - q_sub + 1;
+      CU(ctx->wring.ensure((size_t)nq * P.ntau * P.naux * P.naux * sizeof(double2)));
+      UnfoldParams up;
+      up.src = ctx->dW; up.dst = (double2*)ctx->wring.p;
+      up.tgt_src = (const int*)ctx->tgt_src.p + q_sub; up.tgt_op = (const int*)ctx->tgt_op.p + q_sub;
+      up.colphase = (const double2*)ctx->colphase_aux.p + (size_t)q_sub * P.naux;
+      up.ell_cols = (const int*)ctx->ell_cols_aux.p; up.ell_vals = (const double*)ctx->ell_vals_aux.p;
+      up.ell_cnt = (const int*)ctx->ell_cnt_aux.p;
+      up.n = P.naux; up.ntau = P.ntau; up.maxnz = ctx->maxnz_aux;
+      int rc = tic(ctx, GWSIG_KIND_UNFOLD_W);
+      if (rc) return rc;
+      CU(launch_unfold_sparse(up, nq, ctx->stream));
+      if ((rc = toc(ctx))) return rc;
+      ctx->launches++;
+      Wsrc = (const double2*)ctx->wring.p;
+    }
     for (int t0 = 0; t0 < P.ntau; t0 += nt) {
       const int ntc = std::min(nt, P.ntau - t0);
       DevPlan* dp = nullptr;
-      int rc = get_dev_plan(ctx, s0, ns, ntc, q_first, &dp);
+      int rc = get_dev_plan(ctx, s0, ns, ntc, q_sub, &dp);
       if (rc) return rc;
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Gsrc, Vsub, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]

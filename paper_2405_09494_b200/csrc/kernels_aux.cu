@@ -11,8 +11,8 @@ namespace {
 // O^k(alpha^) = P . diag(ph) is never formed densely: P = (atom permutation) x (real Wigner D) has at
 // most 2l+1 <= 9 entries per row (Eq. 3-4).  X^{k~} = O X^k O^dagger (Eq. 22).
 __global__ void __launch_bounds__(256) unfold_sparse_kernel(UnfoldParams p) {
-  const int tgt = blockIdx.y / p.ntau, t = blockIdx.y % p.ntau;
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  const int tgt = blockIdx.x / p.ntau, t = blockIdx.x % p.ntau;      // (target, tau) on grid.x: Nk * ntau exceeds 65535 at cfg5
+  const int e = blockIdx.y * blockDim.x + threadIdx.x;
   const int n = p.n;
   if (e >= n * n) return;
   const int r = e / n, c = e - r * n;
@@ -130,7 +130,7 @@ __global__ void probe_mixed_kernel(long long iters, double* sink) {
 
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream) {
   if (ntarget <= 0) return cudaSuccess;
-  dim3 grid((unsigned)((p.n * p.n + 255) / 256), (unsigned)(ntarget * p.ntau));
+  dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n * p.n + 255) / 256));
   unfold_sparse_kernel<<<grid, 256, 0, stream>>>(p);
   return cudaGetLastError();
 }

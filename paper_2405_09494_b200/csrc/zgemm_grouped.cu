@@ -1,4 +1,12 @@
-// Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a), engine v3.
+// Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a).
+//
+// TWO tensor-core kernels share the loader, the tile scheduler and the descriptors:
+//   zgemm_grouped_dmma3m (engine 0, default): Karatsuba / "3M" complex product -- three REAL products
+//       P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi),  re = P1 - P2,  im = P3 - P1 - P2  (25 % fewer DMMA than 4M),
+//       one product per group of four MMA warps (12 MMA warps, 32 accumulator doubles each), accumulators handed to
+//       four EPILOGUE warps through shared memory so that the MMA warps never touch global memory or index arithmetic:
+//       loader warps -> MMA warps -> epilogue warps, decoupled by mbarriers (details above the kernel)
+//   zgemm_grouped_dmma   (engine 2): the conventional four-product kernel (engine v3 of round 1), described below.
 //
 // Serves the three contraction stages of the GW self-energy (Algorithm 4 lines 5, 7, 8 of
 // arXiv 2405.09494).  Descriptors: include/gwsig_plan.h.  Design: DESIGN.md section 5.
@@ -21,6 +29,8 @@
 //  * GWSIG_FLAG_ACCUM tiles add into C with red.global.add.f64 (split-K parts of stage 3 share a Sigma block)
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <mutex>
 
 #include "zgemm_grouped.cuh"
 
@@ -120,6 +130,132 @@ constexpr int BK = 8;
 constexpr int LDA = ZG_BM + 2, LDB = ZG_BN + 2;          // = 2 (mod 8): conflict-free fragment loads
 constexpr int kStages = 5;
 static_assert(LDA % 8 == 2 && LDB % 8 == 2, "layout");
+
+// ------------------------------------------------------------------------------------------
+// loader (producer) side, shared by both kernels: kProducerWarps warps stage tiles global -> shared
+// ------------------------------------------------------------------------------------------
+struct RingCtl {
+  unsigned full0, empty0;        // shared addresses of the full / empty mbarrier arrays
+  SlotHdr* hdr;
+  TileRec* trec;
+  int ntrec;
+  long long* next_tile;
+};
+
+__device__ __forceinline__ void producer_loop(const ZgParams& p, double2* As, double2* Bs, const RingCtl& rc, int pw, int lane) {
+  const unsigned full0 = rc.full0, empty0 = rc.empty0;
+  SlotHdr* hdr = rc.hdr;
+  TileRec* trec = rc.trec;
+  long long* next_tile = rc.next_tile;
+  int stage = 0;
+  unsigned phase = 0;
+  const bool leader = pw == 0 && lane == 0;
+  const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
+  int tslot = 0, tbuf = 0;
+  long long pre = 0;                                  // tile id fetched one tile ahead (leader only)
+  if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);
+  while (true) {
+    if (leader) next_tile[tbuf] = pre;
+    named_bar_sync(1, kProducerWarps * 32);
+    const long long tile = next_tile[tbuf];
+    tbuf ^= 1;
+    if (tile >= p.total_tiles) break;
+    if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);       // lands while this tile is being staged
+    const TileInfo ti = decode_tile(p, tile);
+    const gwsig_problem& P = p.prob[ti.prob];
+    const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
+    const int m0 = ti.tm * ZG_BM;
+    int n0, ncols;
+    zg_ntile(N, __ldg(&P.tiles_n), ti.tn, n0, ncols);
+    const int mrows = min(ZG_BM, M - m0);
+    const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
+    const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
+    const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
+    const bool kmajor = (flags & GWSIG_FLAG_A_KMAJOR) != 0;
+    bool first = true;
+    for (int s = 0; s < nseg; ++s) {
+      const gwsig_seg& S = p.seg[seg_begin + s];
+      const int K = __ldg(&S.K);
+      if (K == 0) continue;
+      const bool last_seg = s == nseg - 1;
+      const gwsig_idx2 ak = S.ak, bk = S.bk;
+      const double2* abase = p.A + __ldg(&S.a_off) + a_boff;
+      const bool b_ok = lane < ncols;
+      const double2* b_col = p.B + __ldg(&S.b_off) + b_boff + (b_ok ? idx2(S.bn, n0 + lane) : 0);
+      // A row offsets of this lane (32-bit: element offsets inside a tile stay < 2^31, checked by the plan).
+      //   A contiguous along m: lane <-> tile rows lane + 32 r (r < 4); this warp stages k-rows 2 pw, 2 pw + 1
+      //   A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j, j < 8)
+      const gwsig_idx2 am = S.am;
+      const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
+      int a_roff[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int ml = kmajor ? mr + 16 * j : lane + 32 * j;
+        a_roff[j] = ((kmajor || j < 4) && ml < mrows) ? (int)idx2(am, m0 + ml) : -1;
+      }
+      for (int k0 = 0; k0 < K; k0 += BK) {
+        mbar_wait(empty0 + 8 * stage, phase ^ 1);
+        const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
+        const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
+        const bool two = k0 + 4 < K;                      // the slot's second k4 step holds data
+        if (!kmajor) {
+#pragma unroll
+          for (int h2 = 0; h2 < 2; ++h2) {
+            const int kk = 2 * pw + h2;
+            const int k = k0 + kk;
+            if (kk < 4 || two) {
+              const bool kok = k < K;
+              const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+              for (int r = 0; r < 4; ++r)
+                if (a_roff[r] >= 0) cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, kok ? ap + a_roff[r] : abase, kok);
+            }
+          }
+        } else if (kl < 4 || two) {
+          const int k = k0 + kl;
+          const bool kok = k < K;
+          const double2* ap = abase + (kok ? idx2(ak, k) : 0);
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            if (a_roff[j] >= 0) cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, kok ? ap + a_roff[j] : abase, kok);
+        }
+        if (b_ok) {
+#pragma unroll
+          for (int h2 = 0; h2 < 2; ++h2) {
+            const int kk = 2 * pw + h2;
+            const int k = k0 + kk;
+            if (kk < 4 || two) {
+              const bool kok = k < K;
+              cp_async16(bs + (unsigned)(kk * LDB + lane) * 16u, b_col + (kok ? idx2(bk, k) : 0), kok);
+            }
+          }
+        }
+        mbar_arrive_cp_async(full0 + 8 * stage);
+        if (leader) {                                     // slot header, then a releasing arrive
+          SlotHdr& h = hdr[stage];
+          const bool last = last_seg && k0 + BK >= K;
+          h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
+          h.nk4 = two ? 2 : 1;
+          if (first) {
+            TileRec& t = trec[tslot];
+            t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
+            t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
+            t.cm = P.cm; t.cn = P.cn;
+            h.trec = tslot;
+          }
+          mbar_arrive(full0 + 8 * stage);
+        }
+        if (first) { first = false; if (++tslot == rc.ntrec) tslot = 0; }
+        if (++stage == kStages) { stage = 0; phase ^= 1; }
+      }
+    }
+  }
+  // tell the consumers there is no more work
+  mbar_wait(empty0 + 8 * stage, phase ^ 1);
+  mbar_arrive_cp_async(full0 + 8 * stage);
+  if (leader) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
+  asm volatile("cp.async.wait_all;\n" ::: "memory");
+}
 
 // ------------------------------------------------------------------------------------------
 // consumer side: one warp tile = MI row groups (8 rows each, 32 rows apart) x NI column groups, accumulators
@@ -239,113 +375,9 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
   if (warp >= kConsumerWarps) {
     // ================================= PRODUCERS ================================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kProducerRegs));
-    const int pw = warp - kConsumerWarps;               // producer warp 0..3
-    const bool leader = pw == 0 && lane == 0;
-    const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
-    int tslot = 0, tbuf = 0;
-    long long pre = 0;                                  // tile id fetched one tile ahead (leader only)
-    if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);
-    while (true) {
-      if (leader) next_tile[tbuf] = pre;
-      named_bar_sync(1, kProducerWarps * 32);
-      const long long tile = next_tile[tbuf];
-      tbuf ^= 1;
-      if (tile >= p.total_tiles) break;
-      if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);       // lands while this tile is being staged
-      const TileInfo ti = decode_tile(p, tile);
-      const gwsig_problem& P = p.prob[ti.prob];
-      const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
-      const int m0 = ti.tm * ZG_BM;
-      int n0, ncols;
-      zg_ntile(N, __ldg(&P.tiles_n), ti.tn, n0, ncols);
-      const int mrows = min(ZG_BM, M - m0);
-      const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
-      const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
-      const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
-      const bool kmajor = (flags & GWSIG_FLAG_A_KMAJOR) != 0;
-      bool first = true;
-      for (int s = 0; s < nseg; ++s) {
-        const gwsig_seg& S = p.seg[seg_begin + s];
-        const int K = __ldg(&S.K);
-        if (K == 0) continue;
-        const bool last_seg = s == nseg - 1;
-        const gwsig_idx2 ak = S.ak, bk = S.bk;
-        const double2* abase = p.A + __ldg(&S.a_off) + a_boff;
-        const bool b_ok = lane < ncols;
-        const double2* b_col = p.B + __ldg(&S.b_off) + b_boff + (b_ok ? idx2(S.bn, n0 + lane) : 0);
-        // A row offsets of this lane (32-bit: element offsets inside a tile stay < 2^31, checked by the plan).
-        //   A contiguous along m: lane <-> tile rows lane + 32 r (r < 4); this warp stages k-rows 2 pw, 2 pw + 1
-        //   A contiguous along k: lane <-> (k = lane & 7, tile rows 4 (lane >> 3) + pw + 16 j, j < 8)
-        const gwsig_idx2 am = S.am;
-        const int kl = lane & 7, mr = 4 * (lane >> 3) + pw;
-        int a_roff[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int ml = kmajor ? mr + 16 * j : lane + 32 * j;
-          a_roff[j] = ((kmajor || j < 4) && ml < mrows) ? (int)idx2(am, m0 + ml) : -1;
-        }
-        for (int k0 = 0; k0 < K; k0 += BK) {
-          mbar_wait(empty0 + 8 * stage, phase ^ 1);
-          const unsigned as = as0 + (unsigned)(stage * BK * LDA) * 16u;
-          const unsigned bs = bs0 + (unsigned)(stage * BK * LDB) * 16u;
-          const bool two = k0 + 4 < K;                      // the slot's second k4 step holds data
-          if (!kmajor) {
-#pragma unroll
-            for (int h2 = 0; h2 < 2; ++h2) {
-              const int kk = 2 * pw + h2;
-              const int k = k0 + kk;
-              if (kk < 4 || two) {
-                const bool kok = k < K;
-                const double2* ap = abase + (kok ? idx2(ak, k) : 0);
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                  if (a_roff[r] >= 0) cp_async16(as + (unsigned)(kk * LDA + lane + 32 * r) * 16u, kok ? ap + a_roff[r] : abase, kok);
-              }
-            }
-          } else if (kl < 4 || two) {
-            const int k = k0 + kl;
-            const bool kok = k < K;
-            const double2* ap = abase + (kok ? idx2(ak, k) : 0);
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-              if (a_roff[j] >= 0) cp_async16(as + (unsigned)(kl * LDA + mr + 16 * j) * 16u, kok ? ap + a_roff[j] : abase, kok);
-          }
-          if (b_ok) {
-#pragma unroll
-            for (int h2 = 0; h2 < 2; ++h2) {
-              const int kk = 2 * pw + h2;
-              const int k = k0 + kk;
-              if (kk < 4 || two) {
-                const bool kok = k < K;
-                cp_async16(bs + (unsigned)(kk * LDB + lane) * 16u, b_col + (kok ? idx2(bk, k) : 0), kok);
-              }
-            }
-          }
-          mbar_arrive_cp_async(full0 + 8 * stage);
-          if (leader) {                                     // slot header, then a releasing arrive
-            SlotHdr& h = hdr[stage];
-            const bool last = last_seg && k0 + BK >= K;
-            h.ctl = (first ? 1 : 0) | (last ? 2 : 0);
-            h.nk4 = two ? 2 : 1;
-            if (first) {
-              TileRec& t = trec[tslot];
-              t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
-              t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
-              t.cm = P.cm; t.cn = P.cn;
-              h.trec = tslot;
-            }
-            mbar_arrive(full0 + 8 * stage);
-          }
-          if (first) { first = false; if (++tslot == kStages + 1) tslot = 0; }
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-    // tell the consumers there is no more work
-    mbar_wait(empty0 + 8 * stage, phase ^ 1);
-    mbar_arrive_cp_async(full0 + 8 * stage);
-    if (leader) { hdr[stage].ctl = 4; mbar_arrive(full0 + 8 * stage); }
-    asm volatile("cp.async.wait_all;\n" ::: "memory");
+    RingCtl rc;
+    rc.full0 = full0; rc.empty0 = empty0; rc.hdr = hdr; rc.trec = trec; rc.ntrec = kStages + 1; rc.next_tile = next_tile;
+    producer_loop(p, As, Bs, rc, warp - kConsumerWarps, lane);
   } else {
     // ================================= CONSUMERS ================================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(kConsumerRegs));
@@ -396,6 +428,213 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
 }
 
 // ------------------------------------------------------------------------------------------
+// the 3M kernel: warps 0..11 MMA (three product groups of four), 12..15 loaders, 16..19 epilogue
+//
+//   complex C += A B  as three real products (Karatsuba):  P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi),
+//   re C = P1 - P2,  im C = P3 - P1 - P2.  MMA warp (g, w) accumulates product g for row groups w, w+4, w+8, w+12
+//   of the 128-row tile and all (<= 4) column groups: 32 accumulator doubles.  Warp id mod 4 = w is the SM
+//   sub-partition, so every sub-partition hosts one warp of each product: three independent DMMA streams per FP64
+//   pipe.  conj(A) / conj(B): the sign of Ai / Bi enters the operand sums of P3 (XOR on the integer pipe) and the
+//   sign of P2 in the epilogue.  At the end of a tile the MMA warps drop their accumulators into a shared staging
+//   buffer [3][128][33] and go straight on with the next tile; the epilogue warps combine the three planes, do the
+//   two-level C addressing and store (or red.add) with full-line global accesses in the orientation C is
+//   contiguous in.  Register budget per SM: 12 x 32 x 136 + 4 x 32 x 40 + 4 x 32 x 56 = 64512 <= 65536.
+// ------------------------------------------------------------------------------------------
+constexpr int kMmaWarps = 12;
+constexpr int kEpiWarps = 4;
+constexpr int kMmaRegs = 136, kLoaderRegs3 = 40, kEpiRegs = 56;
+constexpr int kThreads3 = (kMmaWarps + kProducerWarps + kEpiWarps) * 32;
+constexpr int STG_LD = ZG_BN + 1;                      // odd pitch (doubles): conflict-free in both epilogue orientations
+constexpr int kTrec3 = kStages + 3;                    // loaders <= kStages tiles ahead of the MMA warps, epilogue one behind
+
+template <int MI, int NI>
+__device__ __forceinline__ void mma3_k4(double (&acc)[4][4][2], const double2* as, const double2* bs, int grp, unsigned sa,
+                                        unsigned sb) {
+  double2 af[MI], bf[NI];
+  double a[MI], b[NI];
+#pragma unroll
+  for (int i = 0; i < MI; ++i) af[i] = as[i * 32];
+#pragma unroll
+  for (int j = 0; j < NI; ++j) bf[j] = bs[j * 8];
+  if (grp == 0) {
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = af[i].x;
+#pragma unroll
+    for (int j = 0; j < NI; ++j) b[j] = bf[j].x;
+  } else if (grp == 1) {
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = af[i].y;
+#pragma unroll
+    for (int j = 0; j < NI; ++j) b[j] = bf[j].y;
+  } else {
+#pragma unroll
+    for (int i = 0; i < MI; ++i) a[i] = af[i].x + xor_hi(af[i].y, sa);
+#pragma unroll
+    for (int j = 0; j < NI; ++j) b[j] = bf[j].x + xor_hi(bf[j].y, sb);
+  }
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+}
+
+template <int MI, int NI>
+__device__ __forceinline__ void mma3_slot(double (&acc)[4][4][2], const double2* as, const double2* bs, int nk4, int grp,
+                                          unsigned sa, unsigned sb) {
+#pragma unroll 1
+  for (int kk = 0; kk < nk4; ++kk) mma3_k4<MI, NI>(acc, as + kk * 4 * LDA, bs + kk * 4 * LDB, grp, sa, sb);
+}
+
+struct __align__(8) StageCtl {      // handshake MMA warps -> epilogue warps
+  int trec;                          // tile record of the staged tile
+  int ctl;                           // 4: no more tiles
+};
+
+__global__ void __launch_bounds__(kThreads3, 1) zgemm_grouped_dmma3m(ZgParams p) {
+  extern __shared__ double2 zg_smem[];
+  double2* As = zg_smem;                             // [kStages][BK][LDA]
+  double2* Bs = zg_smem + kStages * BK * LDA;        // [kStages][BK][LDB]
+  double* Stg = reinterpret_cast<double*>(zg_smem + kStages * BK * (LDA + LDB));   // [3][ZG_BM][STG_LD]
+  __shared__ __align__(8) unsigned long long bars[2 * kStages + 2];
+  __shared__ SlotHdr hdr[kStages];
+  __shared__ TileRec trec[kTrec3];
+  __shared__ long long next_tile[2];
+  __shared__ StageCtl sctl;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
+  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[kStages]);
+  const unsigned stg_full = (unsigned)__cvta_generic_to_shared(&bars[2 * kStages]);
+  const unsigned stg_empty = (unsigned)__cvta_generic_to_shared(&bars[2 * kStages + 1]);
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, kProducerWarps * 32 + 1); mbar_init(empty0 + 8 * s, kMmaWarps); }
+    mbar_init(stg_full, kMmaWarps);
+    mbar_init(stg_empty, kEpiWarps);
+  }
+  __syncthreads();
+
+  if (warp >= kMmaWarps + kProducerWarps) {
+    // ================================= EPILOGUE WARPS ===========================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kEpiRegs));
+    const int ew = warp - kMmaWarps - kProducerWarps;
+    unsigned tpar = 0;
+    while (true) {
+      mbar_wait(stg_full, tpar);
+      if (sctl.ctl & 4) break;
+      const TileRec& t = trec[sctl.trec];
+      const int mrows = t.mrows, ncols = t.ncols;
+      const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
+      const bool flip = ((t.flags & GWSIG_FLAG_CONJ_A) != 0) != ((t.flags & GWSIG_FLAG_CONJ_B) != 0);   // sign of Ai Bi
+      double2* cbase = p.C + t.c_off;
+      const int row = 32 * ew + lane;
+      const long long my_roff = row < mrows ? idx2(t.cm, t.m0 + row) : -1;
+      const long long my_coff = lane < ncols ? idx2(t.cn, t.n0 + lane) : -1;
+      const double* s1 = Stg, *s2 = Stg + ZG_BM * STG_LD, *s3 = Stg + 2 * ZG_BM * STG_LD;
+      if (t.cm.lo == 1) {
+        // C contiguous along m (X, Y): lane <-> row, walk the columns; 32 lanes write 32 consecutive rows
+        const double* q1 = s1 + row * STG_LD, *q2 = s2 + row * STG_LD, *q3 = s3 + row * STG_LD;
+        for (int c = 0; c < ncols; ++c) {
+          const long long coff = __shfl_sync(0xffffffffu, my_coff, c);
+          if (my_roff >= 0) {
+            const double p1 = q1[c], p2 = flip ? -q2[c] : q2[c], p3 = q3[c];
+            const double re = p1 - p2, im = p3 - p1 - p2;
+            double2* dst = cbase + my_roff + coff;
+            if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
+            else *dst = make_double2(re, im);
+          }
+        }
+      } else {
+        // C contiguous along n (Sigma blocks): lane <-> column, walk this warp's 32 rows
+        const int rend = min(32, mrows - 32 * ew);
+        for (int rr = 0; rr < rend; ++rr) {
+          const long long roff = __shfl_sync(0xffffffffu, my_roff, rr);
+          if (my_coff >= 0) {
+            const int r = 32 * ew + rr;
+            const double p1 = s1[r * STG_LD + lane], p2r = s2[r * STG_LD + lane], p3 = s3[r * STG_LD + lane];
+            const double p2 = flip ? -p2r : p2r;
+            const double re = p1 - p2, im = p3 - p1 - p2;
+            double2* dst = cbase + roff + my_coff;
+            if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
+            else *dst = make_double2(re, im);
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(stg_empty);
+      tpar ^= 1;
+    }
+  } else if (warp >= kMmaWarps) {
+    // ================================= LOADER WARPS =============================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kLoaderRegs3));
+    RingCtl rc;
+    rc.full0 = full0; rc.empty0 = empty0; rc.hdr = hdr; rc.trec = trec; rc.ntrec = kTrec3; rc.next_tile = next_tile;
+    producer_loop(p, As, Bs, rc, warp - kMmaWarps, lane);
+  } else {
+    // ================================= MMA WARPS ================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(kMmaRegs));
+    const int grp = warp >> 2, wq = warp & 3;
+    const int fr = lane >> 2, fk = lane & 3;
+    double acc[4][4][2];
+    int stage = 0, tslot = 0, variant = -1, mi = 0, ng = 0;
+    unsigned phase = 0, tpar = 0, sa = 0, sb = 0;
+    while (true) {
+      mbar_wait(full0 + 8 * stage, phase);
+      const int ctl = hdr[stage].ctl;
+      if (ctl & 4) break;
+      if (ctl & 1) {
+        tslot = hdr[stage].trec;
+        const TileRec& t = trec[tslot];
+        const int mg = (t.mrows + 7) >> 3;
+        ng = (t.ncols + 7) >> 3;
+        mi = mg > wq ? (mg - wq + 3) >> 2 : 0;
+        variant = mi > 0 ? (mi - 1) * 4 + (ng - 1) : -1;
+        sa = (t.flags & GWSIG_FLAG_CONJ_A) ? 0x80000000u : 0u;
+        sb = (t.flags & GWSIG_FLAG_CONJ_B) ? 0x80000000u : 0u;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+      }
+      if (variant >= 0) {
+        const double2* as = As + stage * BK * LDA + fk * LDA + wq * 8 + fr;
+        const double2* bs = Bs + stage * BK * LDB + fk * LDB + fr;
+        const int nk4 = hdr[stage].nk4;
+#define ZG_F(MI_, NI_) mma3_slot<MI_, NI_>(acc, as, bs, nk4, grp, sa, sb);
+        switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
+#undef ZG_F
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+      if (++stage == kStages) { stage = 0; phase ^= 1; }
+
+      if (ctl & 2) {
+        // ---- hand the accumulators of this product to the epilogue warps -----------------------
+        mbar_wait(stg_empty, tpar ^ 1);                 // staging buffer free (passes at once for the first tile)
+        double* sg = Stg + grp * (ZG_BM * STG_LD) + (wq * 8 + fr) * STG_LD + 2 * fk;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (i < mi && j < ng) {
+              sg[i * 32 * STG_LD + j * 8] = acc[i][j][0];
+              sg[i * 32 * STG_LD + j * 8 + 1] = acc[i][j][1];
+            }
+        if (warp == 0 && lane == 0) { sctl.trec = tslot; sctl.ctl = 0; }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(stg_full);
+        tpar ^= 1;
+      }
+    }
+    // no more tiles: release the epilogue warps
+    mbar_wait(stg_empty, tpar ^ 1);
+    if (warp == 0 && lane == 0) sctl.ctl = 4;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(stg_full);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // reference engine: same plan, one thread per output element, plain DFMA, no shared memory
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
@@ -433,6 +672,12 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
 
 }  // namespace
 
+namespace {
+struct LaunchCfg { bool ok3 = false, ok4 = false; int occ4 = 1; };
+LaunchCfg g_cfg[64];                 // per device: the shared-memory opt-in is a per-device function attribute
+std::mutex g_cfg_mu;
+}  // namespace
+
 cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t stream) {
   if (p.total_tiles <= 0) return cudaSuccess;
   if (engine == 1) {
@@ -440,22 +685,40 @@ cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t s
     zgemm_grouped_reference<<<(unsigned)grid, 256, 0, stream>>>(p);
     return cudaGetLastError();
   }
-  // 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 200 / 56 by setmaxnreg
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_cfg_mu);
+  LaunchCfg& cfg = g_cfg[dev];
+  if (engine == 0) {
+    // 3M kernel: 12 MMA + 4 loader + 4 epilogue warps, one persistent CTA per SM
+    constexpr int smem = kStages * BK * (LDA + LDB) * (int)sizeof(double2) + 3 * ZG_BM * STG_LD * (int)sizeof(double);
+    if (!cfg.ok3) {
+      e = cudaFuncSetAttribute(zgemm_grouped_dmma3m, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+      if (e != cudaSuccess) return e;
+      cfg.ok3 = true;
+    }
+    long long grid = num_sms;
+    if (grid > p.total_tiles) grid = p.total_tiles;
+    if (grid < 1) return cudaSuccess;
+    zgemm_grouped_dmma3m<<<(unsigned)grid, kThreads3, smem, stream>>>(p);
+    return cudaGetLastError();
+  }
+  // 4M kernel: 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 200 / 56
   constexpr int smem = kStages * BK * (LDA + LDB) * (int)sizeof(double2);
   constexpr int threads = (kConsumerWarps + kProducerWarps) * 32;
-  static bool configured = false;
-  static int occ = 1;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (!cfg.ok4) {
+    e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zgemm_grouped_dmma, threads, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cfg.occ4, zgemm_grouped_dmma, threads, smem);
     if (e != cudaSuccess) return e;
-    if (occ < 1) occ = 1;
-    configured = true;
+    if (cfg.occ4 < 1) cfg.occ4 = 1;
+    cfg.ok4 = true;
   }
-  long long grid = (long long)num_sms * occ;
+  long long grid = (long long)num_sms * cfg.occ4;
   if (grid > p.total_tiles) grid = p.total_tiles;
   if (grid < 1) return cudaSuccess;
   zgemm_grouped_dmma<<<(unsigned)grid, threads, smem, stream>>>(p);

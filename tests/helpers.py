@@ -7,22 +7,58 @@ from gwsig_synth.group import rep_at_k
 from paper_2405_09494_b200.binding import (FLAG_ACCUM, FLAG_CONJ_A, FLAG_CONJ_B, FULL_BZ, IBZ, IBZ_BLOCK, NODIV)
 
 
+_INPUTS = {}
+_ORACLE = {}
+
+
+def get_inputs(name, **over):
+    """seeded inputs of a config / toy, built once per test session (cfg3 costs ~20 s, cfg5 minutes)."""
+    from gwsig_synth import make_inputs
+    key = (name, tuple(sorted((k, str(v)) for k, v in over.items())))
+    if key not in _INPUTS:
+        _INPUTS[key] = make_inputs(name, **over)
+        _INPUTS[key]._cache_key = key
+    return _INPUTS[key]
+
+
 def oracle_sigma(inp, ks, taus=None):
+    """oracle/sigma_oracle.sigma_ref at the (k, tau) sample -> [len(ks), len(taus), nao, nao].
+
+    The two V tensors of Eq. 16 are generated INDEPENDENTLY (V^{k,k2} by V1_rows, V^{k2,k} by V2_rows; the oracle does
+    not assume the conjugation relation), one batched Bloch sum per sampled k instead of one dense sum per (k, q) call.
+    One k at a time, so the V rows of a single k bound the memory (16 GB at cfg5).  Results are cached per
+    (inputs, k, tau) for the session: tests of different modes on the same sample share one oracle run."""
     from oracle.sigma_oracle import sigma_ref
     taus = np.arange(inp.ntau) if taus is None else np.asarray(taus)
-    cache_g, cache_w = {}, {}
+    nk = inp.nk
+    ckey = getattr(inp, "_cache_key", None)
+    need = [int(k) for k in ks if ckey is None or any((ckey, int(k), int(t)) not in _ORACLE for t in taus)]
+    store = {}
+    if need:
+        Gs = {k: (inp.G_k(k) if hasattr(inp, "G_k") else inp.G_full()[k])[taus] for k in range(nk)}
+        Ws = {q: inp.W_full([q])[0][taus] for q in range(nk)}
+        for k in need:
+            k2s = list(range(nk))
+            rows2 = inp.V2_rows(k, k2s)                    # V^{k2,k}
+            rows1 = inp.V1_rows(k, k2s)                    # V^{k,k2}
 
-    def G_of(k):
-        if k not in cache_g:
-            cache_g[k] = (inp.G_k(k) if hasattr(inp, "G_k") else inp.G_full()[k])[taus]
-        return cache_g[k]
+            diag = [0]
 
-    def W_of(q):
-        if q not in cache_w:
-            cache_w[q] = inp.W_full([q])[0][taus]
-        return cache_w[q]
-
-    return sigma_ref(inp.nk, inp.kmesh.sub, G_of, W_of, inp.V_pair, ks)
+            def V_pair(a, b, k=k, rows1=rows1, rows2=rows2, diag=diag):
+                if a == k and b == k:                      # q = 0: first call is V^{k,k-q}, second V^{k-q,k}
+                    diag[0] ^= 1
+                    return rows1[k] if diag[0] else rows2[k]
+                return rows1[b] if a == k else rows2[a]
+            res = sigma_ref(nk, inp.kmesh.sub, lambda kk: Gs[kk], lambda q: Ws[q], V_pair, [k])[0]
+            del rows1, rows2
+            for b, t in enumerate(taus):
+                store[(k, int(t))] = res[b]
+                if ckey is not None:
+                    _ORACLE[(ckey, k, int(t))] = res[b]
+    out = []
+    for k in ks:
+        out.append(np.stack([store[(int(k), int(t))] if (int(k), int(t)) in store else _ORACLE[(ckey, int(k), int(t))] for t in taus]))
+    return np.stack(out)
 
 
 def fold_to_orbital(cfg, inp, sigma_list):

@@ -4,8 +4,7 @@ FP64, after folding the result back to the orbital basis."""
 import numpy as np
 import pytest
 
-from gwsig_synth import make_inputs
-from tests.helpers import fold_to_orbital, oracle_sigma, rel_err
+from tests.helpers import fold_to_orbital, get_inputs, oracle_sigma, rel_err
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -69,19 +68,19 @@ def _setup(name, mode, **over):
     from paper_2405_09494_b200.pack import Configured, configure_from_crystal
     lib = B.Gwsig(device=0)
     if name == "cfg1":
-        inp = make_inputs("cfg1", **over)
+        inp = get_inputs("cfg1", **over)
         cfg = Configured(lib, mode, np.eye(3), inp.kmesh.N, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
         Gf, Wf = inp.G_full(), inp.W_full()
         G, W = cfg.pack_GW(lambda k: Gf[k], lambda q: Wf[q])
     else:
-        inp = make_inputs(name, **over)
+        inp = get_inputs(name, **over)
         cfg = configure_from_crystal(lib, inp.cr, mode)
         G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
     V = cfg.pack_V(inp.V2_rows)
     return B, inp, cfg, G, W, V
 
 
-@pytest.mark.parametrize("engine", [1, 0])
+@pytest.mark.parametrize("engine", [1, 0, 2])
 def test_cfg1_full_bz(engine):
     """BASELINE.json config 1, whole output."""
     B, inp, cfg, G, W, V = _setup("cfg1", 0)
@@ -99,7 +98,7 @@ def test_cfg1_ragged_and_chunked():
 @pytest.mark.parametrize("mode", [1, 2])
 def test_toys_ibz_and_block(name, mode):
     B, inp, cfg, G, W, V = _setup(name, mode)
-    for engine in (1, 0):
+    for engine in (1, 0, 2):
         _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
     _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=1))
 
@@ -116,7 +115,7 @@ def _setup_full_from_crystal(name):
     """FULL_BZ mode on a crystal: inputs given on the whole mesh, no symmetry passed."""
     B = _B()
     from paper_2405_09494_b200.pack import Configured
-    inp = make_inputs(name)
+    inp = get_inputs(name)
     cr = inp.cr
     lib = B.Gwsig(device=0)
     cfg = Configured(lib, 0, cr.a, cr.mesh, cr.nao, cr.naux, cr.ntau, cr.beta, None, None, None)
@@ -130,7 +129,7 @@ def _sampled(name, mode, pick, taus, pushes_q=None):
     independent sum over all q, gwsig_set_output_points), all tau on the GPU, oracle at the sampled tau."""
     B = _B()
     from paper_2405_09494_b200.pack import configure_from_crystal
-    inp = make_inputs(name)
+    inp = get_inputs(name)
     lib = B.Gwsig(device=0)
     cfg = configure_from_crystal(lib, inp.cr, mode, out_points=pick)
     G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
@@ -138,6 +137,52 @@ def _sampled(name, mode, pick, taus, pushes_q=None):
     sig = run_gpu(cfg, G, W, V, pushes=None if pushes_q is None else pushes_q * cfg.nk1)
     w = _check(cfg, inp, sig, ks=[int(k) for k in cfg.out_list], taus=taus)
     print(name, "mode", mode, "points", list(cfg.out_list), "tau", list(taus), "worst rel err", w)
+
+
+def _variants_hit(cfg):
+    """(row groups, column groups) per MMA warp that the tiles of all three stages produce: the engine instantiates its
+    main loop for each of the 16 combinations (zgemm_grouped.cu, ZG_VARIANTS).  Tiling rule of zgemm_grouped.cuh restated."""
+    hit = set()
+    for stage in (1, 2, 3):
+        prob, _, _ = cfg.lib.plan_get(0, cfg.npairs, cfg.ntau, stage)
+        for P in prob:
+            M, N = int(P["M"]), int(P["N"])
+            G = (N + 7) // 8
+            tn = (G + 3) // 4
+            ngs = {((j + 1) * G) // tn - (j * G) // tn for j in range(tn)}
+            for m0 in range(0, M, 128):
+                mg = (min(128, M - m0) + 7) // 8
+                for wq in range(4):
+                    if mg > wq:
+                        hit |= {((mg - wq + 3) // 4, ng) for ng in ngs}
+    return hit
+
+
+_VARIANT_CASES = [(7, 5, 2), (10, 13, 3), (10, 21, 2), (12, 29, 3), (5, 27, 13), (3, 9, 37)]
+
+
+def test_engine_variants_are_all_exercised():
+    """every (row groups, column groups) variant of the tensor kernels' main loop, ragged M / N / K tails in all stages:
+    small no-symmetry problems whose nao / naux / ntau are chosen so that the union of their tiles covers all 16."""
+    hit = set()
+    for nao, naux, ntau in _VARIANT_CASES:
+        B, inp, cfg, G, W, V = _setup("cfg1", 0, mesh=(2, 1, 1), nao=nao, naux=naux, ntau=ntau, beta=3.0, nocc=max(1, nao // 2), seed=nao)
+        hit |= _variants_hit(cfg)
+        for engine in (0, 2):
+            _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
+    assert hit == {(mi, ni) for mi in range(1, 5) for ni in range(1, 5)}, sorted(hit)
+
+
+def test_cfg3_shaped_small_mesh_full_oracle():
+    """BASELINE configs[2]'s real shell lists (nao 26, naux 116: cfg3's irrep block sizes, N not a multiple of 8, K not a
+    multiple of 4, stage-3 segment lists cut along P') on a 2x2x2 mesh with 5 tau points, where the oracle can check EVERY
+    (k, tau) of the zone: block mode with both tensor kernels, IBZ mode, several pushes and tau chunks."""
+    B, inp, cfg, G, W, V = _setup("cfg3", 2, mesh=(2, 2, 2), ntau=5)
+    for engine in (0, 2):
+        _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
+    _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=2))
+    B, inp, cfg, G, W, V = _setup("cfg3", 1, mesh=(2, 2, 2), ntau=5)
+    _check(cfg, inp, run_gpu(cfg, G, W, V))
 
 
 def test_output_point_subset_matches_full_run():
@@ -153,17 +198,24 @@ def test_output_point_subset_matches_full_run():
 
 
 def test_cfg3_sampled():
+    """BASELINE configs[2] at full size: block mode at three wedge points of different little-group order (Gamma, a
+    line point, a generic point), IBZ mode (unfold kernels, W ring, several pushes) at one of them."""
     _sampled("cfg3", 2, lambda wedge: [wedge[0], wedge[5], wedge[-1]], [0, 51, 103])
-    _sampled("cfg3", 1, lambda wedge: [wedge[3]], [7], pushes_q=54)
+    _sampled("cfg3", 1, lambda wedge: [wedge[5]], [51], pushes_q=54)
 
 
 def test_cfg4_sampled():
+    """BASELINE configs[3] (wurtzite, 12 operations, nonsymmorphic), P9 sample: 2 wedge points x 2 tau in block mode,
+    one of them again in IBZ mode with several pushes (the oracle run is shared)."""
     _sampled("cfg4", 2, lambda wedge: [wedge[0], wedge[9]], [0, 127])
-    _sampled("cfg4", 1, lambda wedge: [wedge[-1]], [64], pushes_q=24)
+    _sampled("cfg4", 1, lambda wedge: [wedge[9]], [127], pushes_q=24)
 
 
 def test_cfg5_sampled():
+    """BASELINE configs[4] (rock salt, 8x8x8): block mode at Gamma and at the last wedge point, IBZ mode (Nk * ntau =
+    69632 unfold targets: beyond a 65535 grid.y) at the last wedge point."""
     _sampled("cfg5", 2, lambda wedge: [wedge[0], wedge[-1]], [0, 135])
+    _sampled("cfg5", 1, lambda wedge: [wedge[-1]], [135], pushes_q=64)
 
 
 def test_hermitize_option_and_observed_hermiticity():
