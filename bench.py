@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-sample-tau", type=int, default=4, help="tau points of the oracle sample")
+    ap.add_argument("--ibz-nq", type=int, default=0, help="q slices timed in the IBZ comparison leg (0: all; 16 at cfg4/cfg5), scaled")
+    ap.add_argument("--full-nq", type=int, default=0, help="q slices timed in the FULL_BZ comparison leg (0: 8; 2 at cfg4/cfg5), scaled")
     ap.add_argument("--engine", type=int, default=0, choices=[0, 2], help="0: DMMA 3M kernel (default), 2: DMMA 4M kernel")
     ap.add_argument("--probe-only", action="store_true", help="print the FP64 issue-rate probes and exit")
     return ap.parse_args()
@@ -106,33 +108,48 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # workload: seeded synthetic inputs (gwsig_synth) laid out for one mode of the library
 # ------------------------------------------------------------------------------------------------
-def device_bloch_V2(inp, k2s, k1s, torch, dev, batch=512):
+class DeviceV:
     """INPUT GENERATION (not the hot path): the generator's Bloch sum (gwsig_synth.tensors.SymmetricInputs.V2_rows),
-    V^{k2,k1}_{Q,bj} = sum_{R1,R2} e^{-2 pi i k2.R1 + 2 pi i k1.R2} V_{Q,b,j}(R1,R2), for a list of (k2, k1) pairs, done
-    with torch on the device because the dense legs need thousands of pairs.  Checked against the numpy generator on
-    sampled pairs by the caller.  Returns a device tensor [npair, naux*nao*nao]."""
-    Vd = torch.from_numpy(inp.Vd.reshape(len(inp.vR1) * len(inp.vR2), -1)).to(dev).to(torch.complex128)
-    fr = inp.kmesh.frac
-    out = torch.empty((len(k1s), Vd.shape[1]), dtype=torch.complex128, device=dev)
-    for s in range(0, len(k1s), batch):
-        a2, a1 = np.asarray(k2s[s:s + batch]), np.asarray(k1s[s:s + batch])
+    V^{k2,k1}_{Q,bj} = sum_{R1,R2} e^{-2 pi i k2.R1 + 2 pi i k1.R2} V_{Q,b,j}(R1,R2), for lists of (k2, k1) pairs, done with
+    torch on the device because a step needs thousands of pairs (and at config 5 they cannot all be resident: the compact
+    real-space table is, 15 GB).  Two real GEMMs against the REAL table.  Pinned to the numpy generator by check()."""
+
+    def __init__(self, inp, torch, dev):
+        self.inp, self.torch, self.dev = inp, torch, dev
+        self.Vd = torch.from_numpy(inp.Vd.reshape(len(inp.vR1) * len(inp.vR2), -1)).to(dev)      # real [nR1 nR2, nel]
+        self.nel = self.Vd.shape[1]
+
+    def dense(self, k2s, k1s):
+        torch, inp = self.torch, self.inp
+        fr = inp.kmesh.frac
+        a2, a1 = np.asarray(k2s), np.asarray(k1s)
         f1 = np.exp(-2j * np.pi * (fr[a2] @ inp.vR1.T))              # [n, nR1]
         f2 = np.exp(+2j * np.pi * (fr[a1] @ inp.vR2.T))              # [n, nR2]
         F = (f1[:, :, None] * f2[:, None, :]).reshape(len(a1), -1)
-        out[s:s + len(a1)] = torch.from_numpy(F).to(dev) @ Vd
-    del Vd
-    return out
+        Fr, Fi = torch.from_numpy(np.ascontiguousarray(F.real)).to(self.dev), torch.from_numpy(np.ascontiguousarray(F.imag)).to(self.dev)
+        return torch.complex(Fr @ self.Vd, Fi @ self.Vd)               # [n, naux*nao*nao]
+
+    def check(self, k2s, k1s, V):
+        for p in sorted({0, len(k1s) // 2, len(k1s) - 1}):
+            ref = self.inp.V2_rows(int(k1s[p]), [int(k2s[p])])[0].ravel()
+            got = V[p].reshape(-1).cpu().numpy()
+            assert np.abs(got - ref).max() <= 1e-12 * max(np.abs(ref).max(), 1e-300), "device V synthesis disagrees with the generator"
 
 
 class Workload:
-    """inputs of one (config, mode): host arrays in the library's layout, plus what the oracle needs."""
+    """inputs of one (config, mode) in the library's layout.  G, W: host arrays (device tensor for the parts that are
+    only ever zero).  V: resident on the device when it fits (packed blocks in IBZ_BLOCK mode, Eq. 27 done by
+    presetup_device on the GPU), else synthesised per batch of whole q into one device slot inside the step ("V is copied
+    on demand": here it is re-derived on demand from the compact real-space table)."""
 
-    def __init__(self, name, mode, B, pack, inp=None, nq_subset=None, torch=None, dev=None, device_index=0, host_only=False):
+    def __init__(self, name, mode, B, pack, inp=None, nq_subset=None, torch=None, dev=None, device_index=0, host_only=False,
+                 resident_limit_gb=110.0, q_per_batch=None):
         from gwsig_synth import make_inputs
-        self.name, self.mode = name, mode
+        self.name, self.mode, self.torch, self.dev = name, mode, torch, dev
         self.inp = inp if inp is not None else make_inputs(name)
         inp = self.inp
         self.lib = B.Gwsig(device=-1 if host_only else device_index)
+        nq_ = None
         if name == "cfg1":
             self.cfg = pack.Configured(self.lib, mode, np.eye(3), inp.kmesh.N, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
             Gf, Wf = inp.G_full(), inp.W_full()
@@ -141,42 +158,122 @@ class Workload:
             cr = inp.cr
             self.cfg = pack.Configured(self.lib, mode, cr.a, cr.mesh, cr.nao, cr.naux, cr.ntau, cr.beta, None, None, None)
             nq_ = cr.kmesh.nk if nq_subset is None else nq_subset          # W(q) of q slices that are never pushed is never read
-            zero_w = np.zeros((cr.ntau, cr.naux, cr.naux), complex)
-            G_of, W_of = inp.G_k, (lambda q: inp.W_full([q])[0] if q < nq_ else zero_w)
+            G_of, W_of = inp.G_k, (lambda q: inp.W_full([q])[0])
         else:
             self.cfg = pack.configure_from_crystal(self.lib, inp.cr, mode)
             G_of, W_of = inp.G_k, (lambda q: inp.W_full([q])[0])
         cfg = self.cfg
-        self.G, self.W = cfg.pack_GW(G_of, W_of)
+        if nq_ is not None and nq_ < cfg.nk:
+            # FULL_BZ on a q subset: only W(q < nq) is ever read; the rest of the [Nk] buffer stays zero on the device (100 GB at cfg5)
+            self.G = np.ascontiguousarray(np.stack([G_of(int(k)) for k in range(cfg.nk)]).ravel(), np.complex128)
+            Wpart = np.ascontiguousarray(np.stack([W_of(int(q)) for q in range(nq_)]).ravel(), np.complex128)
+            self.W = torch.zeros(self.lib.buffer_sizes()[1], dtype=torch.complex128, device=dev)
+            self.W[:Wpart.size] = torch.from_numpy(Wpart).to(dev)
+        else:
+            self.G, self.W = cfg.pack_GW(G_of, W_of)
         self.nq = cfg.nk if nq_subset is None else min(nq_subset, cfg.nk)      # q slices actually pushed
         self.npairs_run = self.nq * cfg.nk1
+        self.resident = True
+        self.setup_notes = {}
         if name == "cfg1" or torch is None:
             self.V = cfg.pack_V(inp.V2_rows)
         else:
-            # dense V2 for the pairs that will be pushed, synthesised on the device (input generation)
-            k1s = [int(cfg.out_list[p % cfg.nk1]) for p in range(self.npairs_run)]
-            k2s = [int(inp.kmesh.sub(k1s[p], p // cfg.nk1)) for p in range(self.npairs_run)]
-            Vdev = device_bloch_V2(inp, k2s, k1s, torch, dev)
-            chk = [0, self.npairs_run // 2, self.npairs_run - 1]
-            for p in chk:                                                      # pin the device synthesis to the numpy generator
-                ref = inp.V2_rows(k1s[p], [k2s[p]])[0].ravel()
-                got = Vdev[p].cpu().numpy()
-                assert np.abs(got - ref).max() <= 1e-12 * max(np.abs(ref).max(), 1e-300), "device V synthesis disagrees with the generator"
-            if mode == B.IBZ_BLOCK:
-                Vh = Vdev.cpu().numpy().reshape(self.npairs_run, inp.naux, inp.nao, inp.nao)
-                del Vdev
-                row_of = {}
-                for p in range(self.npairs_run):
-                    row_of[(k1s[p], k2s[p])] = p
-                self.V = cfg.pack_V(lambda k1, k2list: np.stack([Vh[row_of[(k1, int(k2))]] for k2 in k2list]))
-                del Vh
-            else:
-                self.V = Vdev.reshape(-1)                                        # stays on the device
+            self._device_V(B, resident_limit_gb, q_per_batch)
         self.full_equiv, self.executed = self.lib.flop_counts()
-        if self.nq != cfg.nk:
-            self.executed_run = self.executed * self.nq / cfg.nk
+        self.executed_run = self.executed * self.nq / cfg.nk if self.nq != cfg.nk else self.executed
+
+    # ---- V on the device ---------------------------------------------------------------------------------
+    def _pairs(self, p0, p1):
+        cfg = self.cfg
+        k1s = [int(cfg.out_list[p % cfg.nk1]) for p in range(p0, p1)]
+        qs = [p // cfg.nk1 for p in range(p0, p1)]
+        k2s = [int(self.inp.kmesh.sub(k1, q)) for k1, q in zip(k1s, qs)]
+        return qs, k2s, k1s
+
+    def _device_V(self, B, resident_limit_gb, q_per_batch):
+        torch, dev, cfg, lib = self.torch, self.dev, self.cfg, self.lib
+        t0 = time.time()
+        self.dv = DeviceV(self.inp, torch, dev)
+        nel = self.dv.nel
+        nk1 = cfg.nk1
+        qb = q_per_batch or max(1, int(2.0e9 // (nk1 * nel * 16)))            # ~2 GB of dense V per generation batch
+        self.batches = [(q0 * nk1, min(q0 + qb, self.nq) * nk1) for q0 in range(0, self.nq, qb)]
+        blockmode = self.mode == B.IBZ_BLOCK
+        if blockmode:
+            from paper_2405_09494_b200.presetup_device import DeviceBlocker
+            self.blk = DeviceBlocker(cfg, torch, dev)
+            # pass 1 (pre-step, all pairs of the mode: set_triples wants every pair): allowed blocks by block max-abs
+            trip, vmax = [], None
+            allb = [(q0 * nk1, min(q0 + qb, cfg.nk) * nk1) for q0 in range(0, cfg.nk, qb)]
+            for bi, (p0, p1) in enumerate(allb):
+                qs, k2s, k1s = self._pairs(p0, p1)
+                V = self.dv.dense(k2s, k1s)
+                if bi == 0:
+                    self.dv.check(k2s, k1s, V)
+                    vmax = float(V.abs().max())
+                T = self.blk.transform(V.reshape(len(k1s), cfg.naux, cfg.nao, cfg.nao), qs, k2s, k1s)
+                del V
+                trip += self.blk.triples_from_maxabs(self.blk.block_maxabs(T, qs, k2s, k1s), qs, k2s, k1s, 1e-9, vmax)
+                del T
+            tptr = np.zeros(cfg.npairs + 1, np.int64)
+            tptr[1:] = np.cumsum([len(t) for t in trip])
+            lib.set_triples(tptr, np.concatenate(trip))
+            cfg.triple_ptr, cfg.triples = tptr, trip
+            self.tables = []
+            for (p0, p1) in self.batches:
+                qs, k2s, k1s = self._pairs(p0, p1)
+                self.tables.append(self.blk.pack_tables(trip[p0:p1], qs, k2s, k1s))
+            sizes = np.concatenate([t[3] for t in self.tables])
+            assert all(int(sizes[i]) == lib.pair_info(i)[4] for i in (0, len(sizes) // 2, len(sizes) - 1)), "packed V layout mismatch"
+            self.voff = np.concatenate([[0], np.cumsum(sizes)])
         else:
-            self.executed_run = self.executed
+            self.voff = np.arange(self.npairs_run + 1, dtype=np.int64) * nel
+        total_gb = float(self.voff[-1]) * 16 / 1e9
+        self.resident = total_gb <= resident_limit_gb
+        self.setup_notes = {"v_total_gb": round(total_gb, 2), "v_resident": self.resident, "q_per_generation_batch": qb}
+        if self.resident:
+            self.V = torch.empty(int(self.voff[-1]), dtype=torch.complex128, device=dev)
+            for bi in range(len(self.batches)):
+                self.fill(bi, self.V, int(self.voff[self.batches[bi][0]]), check=(bi == 0 and not blockmode))
+        else:
+            slot = max(int(self.voff[p1] - self.voff[p0]) for p0, p1 in self.batches)
+            self.V = None
+            self.slot = torch.empty(slot, dtype=torch.complex128, device=dev)
+        self.setup_notes["v_setup_s"] = round(time.time() - t0, 1)
+
+    def fill(self, bi, dst, base, check=False):
+        """dense Bloch sum (+ Eq. 27 transform and packing in block mode) of generation batch bi into dst[base:]."""
+        p0, p1 = self.batches[bi]
+        qs, k2s, k1s = self._pairs(p0, p1)
+        V = self.dv.dense(k2s, k1s)
+        if check:
+            self.dv.check(k2s, k1s, V)
+        if self.mode == 2:
+            cfg = self.cfg
+            T = self.blk.transform(V.reshape(len(k1s), cfg.naux, cfg.nao, cfg.nao), qs, k2s, k1s)
+            del V
+            self.blk.pack(T, qs, k2s, k1s, self.tables[bi], dst, (self.voff[p0:p1] - self.voff[p0]) + base)
+        else:
+            dst[base:base + V.numel()] = V.reshape(-1)
+
+    def evaluate(self, dG, dW, dS, stream, dV=None):
+        """enqueue ONE evaluation: resident V -> sigma_eval; otherwise begin / per batch {synthesise into the slot, push} / end."""
+        lib, cfg = self.lib, self.cfg
+        partial = self.npairs_run != cfg.npairs
+        if self.resident and not partial:
+            lib.sigma_eval(dG, dV, dW, dS, stream)
+            return
+        lib.sigma_begin(dG, dW, dS, stream)
+        if self.resident:
+            lib.sigma_push_pairs(0, self.npairs_run, dV)
+        else:
+            for bi, (p0, p1) in enumerate(self.batches):
+                self.fill(bi, self.slot, 0)                       # same stream: the slot is rewritten after the previous push drained
+                lib.sigma_push_pairs(p0, p1 - p0, self.slot)
+        if partial:
+            lib.sigma_abort()
+        else:
+            lib.sigma_end()
 
 
 def stage_flops(wl, B):
@@ -200,32 +297,23 @@ def to_dev(x, torch, dev):
     return x if torch.is_tensor(x) else torch.from_numpy(x).to(dev)
 
 
-def run_resident(wl, torch, dev, steps, warmup, timing=True):
-    """K evaluations with G, W, V resident in HBM; device time by CUDA events on the launching stream.
+def run_steps(wl, torch, dev, steps, warmup, timing=True):
+    """K evaluations (G, W and -- when it fits -- V resident in HBM); device time by CUDA events on the launching stream.
     Returns (seconds per step list, per-kind kernel times of the last step, launches per step, dSigma)."""
-    lib, cfg = wl.lib, wl.cfg
-    dG, dW, dV = to_dev(wl.G, torch, dev), to_dev(wl.W, torch, dev), to_dev(wl.V, torch, dev)
+    lib = wl.lib
+    dG, dW = to_dev(wl.G, torch, dev), to_dev(wl.W, torch, dev)
+    dV = to_dev(wl.V, torch, dev) if wl.V is not None else None
     dS = torch.zeros(lib.buffer_sizes()[2], dtype=torch.complex128, device=dev)
     stream = torch.cuda.current_stream().cuda_stream
     lib.set_option("timing", 1 if timing else 0)
-    partial = wl.npairs_run != cfg.npairs
-
-    def once():
-        if not partial:
-            lib.sigma_eval(dG, dV, dW, dS, stream)
-        else:
-            lib.sigma_begin(dG, dW, dS, stream)
-            lib.sigma_push_pairs(0, wl.npairs_run, dV)
-            lib.sigma_abort()
-
     for _ in range(warmup):
-        once()
+        wl.evaluate(dG, dW, dS, stream, dV)
     torch.cuda.synchronize()
     times = []
     for _ in range(steps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        once()
+        wl.evaluate(dG, dW, dS, stream, dV)
         e1.record()
         e1.synchronize()
         times.append(e0.elapsed_time(e1) * 1e-3)
@@ -389,18 +477,19 @@ def main():
     t_setup = time.time() - t_setup
 
     # ---- the timed region: W warm-up steps, then exactly K steps between barrier + synchronize --------------
-    dG, dW, dV = to_dev(wl.G, torch, dev), to_dev(wl.W, torch, dev), to_dev(wl.V, torch, dev)
+    dG, dW = to_dev(wl.G, torch, dev), to_dev(wl.W, torch, dev)
+    dV = to_dev(wl.V, torch, dev) if wl.V is not None else None
     dS = torch.zeros(lib.buffer_sizes()[2], dtype=torch.complex128, device=dev)
     stream = torch.cuda.current_stream().cuda_stream
     lib.set_option("timing", 1)
     for _ in range(args.warmup):
-        lib.sigma_eval(dG, dV, dW, dS, stream)
+        wl.evaluate(dG, dW, dS, stream, dV)
     barrier()
     sampler = ClockSampler(local)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        lib.sigma_eval(dG, dV, dW, dS, stream)
+        wl.evaluate(dG, dW, dS, stream, dV)
     e1.record()
     barrier()
     secs = e0.elapsed_time(e1) * 1e-3
@@ -412,7 +501,7 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         secs = float(t.item())
     sigma_gpu = dS.cpu().numpy()
-    del dV
+    dV = None
     ms_step = secs / args.steps * 1e3
     ms_eval = ms_step / world                      # replicas: `world` evaluations finish per step time
 
@@ -421,7 +510,10 @@ def main():
             "dtype": "complex128 (f64)", "data": "synthetic",
             "config": {"workload": f"{args.workload} ({describe(args.workload)})", "mode": args.mode, "engine": {0: "dmma 3M", 2: "dmma 4M"}[args.engine], "nk": int(cfg.nk), "nik": int(cfg.nk1),
                        "nao": int(cfg.nao), "naux": int(cfg.naux), "ntau": int(cfg.ntau), "pairs": int(cfg.npairs),
-                       "l2": "inputs larger than L2 (V alone is %.2f GB)" % (wl.V.numel() * 16 / 1e9 if torch.is_tensor(wl.V) else wl.V.nbytes / 1e9),
+                       "l2": "inputs larger than L2 (V alone is %.2f GB)" % (wl.setup_notes.get("v_total_gb") or wl.V.nbytes / 1e9),
+                       "v": ("resident in HBM" if wl.resident else "synthesised on the device per batch of whole q INSIDE the step (all pairs do not fit HBM): "
+                             "value includes that input generation, kernels_last_step is the library alone"),
+                       **wl.setup_notes,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": round(t_setup, 1)},
             "gpu_launches": int(launches) * args.steps, "clocks": clocks}
     if rank != 0:
@@ -441,15 +533,20 @@ def main():
                            "frac_fp64_tensor_peak": (sf[0] + sf[1] + sf[2]) / max(t1 + t2 + t3, 1e-12) / 1e12 / peak,
                            "stage_tflops": [sf[0] / max(t1, 1e-12) / 1e12, sf[1] / max(t2, 1e-12) / 1e12, sf[2] / max(t3, 1e-12) / 1e12],
                            "stage_gflop": [x / 1e9 for x in sf]}
+    probe_tf = max(lib.probe_fp64(0, w, b, 20000)[0] for w, b in ((8, 2), (16, 2)))
     dom = int(np.argmax([t1, t2, t3]))
     ach = sf[dom] / max((t1, t2, t3)[dom], 1e-12) / 1e12
     line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + (" (zgemm_grouped_dmma3m)" if args.engine == 0 else " (zgemm_grouped_dmma)"),
                         "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
-                        "peak_source": "FP64 tensor (DMMA) peak derived from unit counts x max clock, 148 x 128 flop/clk x 1.965 GHz; "
-                                       "the register-only DMMA probe of this library reaches 36.9 (MEASURED_PEAKS.json has no FP64 entry)"}
+                        "peak_measured_dmma_probe": probe_tf,
+                        "peak_source": "FP64 tensor (DMMA) peak derived from unit counts x max clock, 148 x 128 flop/clk x 1.965 GHz "
+                                       "(MEASURED_PEAKS.json has no FP64 entry); peak_measured_dmma_probe is the register-only DMMA issue-rate "
+                                       "probe of this library (gwsig_probe_fp64) run in this job",
+                        "note": "achieved counts ALGORITHMIC flops (8 per complex multiply-add); the 3M kernel executes 6 per complex "
+                                "multiply-add on the pipe, so a fully busy pipe would read 1.33"}
 
     # ---- end to end through the host-buffer call ------------------------------------------------------------------
-    if not args.no_e2e:
+    if not args.no_e2e and wl.resident and wl.setup_notes.get("v_total_gb", 0) <= 16:
         et, h2d, d2h, hs = run_e2e(wl, torch, dev, args.steps, max(1, min(args.warmup, 2)))
         line["e2e"] = {"value": float(np.mean(et)) * 1e3, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                        "api": "gwsig_sigma_eval_host (pinned host G, W, V -> host Sigma; V streamed through a 2-slot ring)"}
@@ -471,13 +568,17 @@ def main():
     # ---- speedup of symmetry adaptation: the other modes on the same crystal, all on the GPU ----------------------
     if not args.no_modes and args.workload != "cfg1":
         modes = {args.mode: {"ms": ms_eval, "gflop_executed": wl.executed / 1e9}}
-        del wl.V
+        wl.V = None
+        if hasattr(wl, "slot"):
+            del wl.slot
         torch.cuda.empty_cache()
-        for mname, nq in (("ibz", None), ("full_bz", 8)):
+        big = args.workload in ("cfg4", "cfg5")
+        for mname, nq in (("ibz", args.ibz_nq or (16 if big else None)), ("full_bz", args.full_nq or (2 if big else 8))):
             if mname == args.mode:
                 continue
             w2 = Workload(args.workload, MODES[mname], B, pack, inp=wl.inp, nq_subset=nq, torch=torch, dev=dev, device_index=local)
-            tt, _, _, _ = run_resident(w2, torch, dev, 1, 1, timing=False)
+            w2.lib.set_option("engine", args.engine)
+            tt, _, _, _ = run_steps(w2, torch, dev, 1, 1, timing=False)
             scale = w2.cfg.nk / w2.nq
             modes[mname] = {"ms": tt[0] * 1e3 * scale, "gflop_executed": w2.executed / 1e9}
             if scale != 1:

@@ -209,12 +209,13 @@ def average_two_index(cr: Crystal, Xr: dict, P: np.ndarray, start: np.ndarray) -
 def average_three_index(cr: Crystal, Vr: dict) -> dict:
     """(1/|G|) sum_g g.V with
     (g.V)_{(pi(z)Q'),(pi(x)i'),(pi(y)j')}(W R1 + s_x - s_z, W R2 + s_y - s_z)
-        += Daux_{Q'Q} D_{i'i} D_{j'j} V_{Q,i,j}(R1,R2)                                (G8)."""
+        += Daux_{Q'Q} D_{i'i} D_{j'j} V_{Q,i,j}(R1,R2)                                (G8).
+    Returns (keys, blocks) rather than a dict: the table is 15 GB at config 5."""
     klist = list(Vr.keys())
     keys = np.array([list(k[0]) + list(k[1]) for k in klist], dtype=np.int64)
     M = np.stack([Vr[k] for k in klist])
     ok, om = _group_average(cr, keys, M, (cr.P_aux, cr.P_ao, cr.P_ao), (cr.aux_start, cr.ao_start, cr.ao_start), 3)
-    return {(tuple(int(v) for v in k[:3]), tuple(int(v) for v in k[3:])): m for k, m in zip(ok, om)}
+    return [tuple(int(v) for v in k) for k in ok], om          # keys (R1, R2) as 6-tuples, blocks [n, naux, nao, nao]
 
 
 def _cdot_real(f: np.ndarray, X: np.ndarray, axis: int) -> np.ndarray:
@@ -258,18 +259,19 @@ class SymmetricInputs:
                 raw[(tuple(R1), tuple(R2))] = (r.standard_normal((cr.naux, cr.nao, cr.nao))
                                                * np.exp(-(d1_ + d2_) / d1) / np.sqrt(cr.naux))
         raw = {K: 0.5 * (M + raw[(K[1], K[0])].transpose(0, 2, 1)) for K, M in raw.items()}
-        Vr = average_three_index(cr, raw)
+        vkeys, vvals = average_three_index(cr, raw)
+        del raw
         # dense [nR1, nR2, naux*nao*nao] table for fast Bloch sums
-        self.vR1 = sorted({K[0] for K in Vr})
-        self.vR2 = sorted({K[1] for K in Vr})
+        R1s, R2s = [tuple(k[:3]) for k in vkeys], [tuple(k[3:]) for k in vkeys]
+        self.vR1 = sorted(set(R1s))
+        self.vR2 = sorted(set(R2s))
         i1 = {R: i for i, R in enumerate(self.vR1)}
         i2 = {R: i for i, R in enumerate(self.vR2)}
         self.Vd = np.zeros((len(self.vR1), len(self.vR2), cr.naux * cr.nao * cr.nao))
-        for (R1, R2), M in Vr.items():
-            self.Vd[i1[R1], i2[R2]] = M.ravel()
+        self.Vd[[i1[R] for R in R1s], [i2[R] for R in R2s]] = vvals.reshape(len(vvals), -1)
+        del vvals
         self.vR1 = np.array(self.vR1)
         self.vR2 = np.array(self.vR2)
-        self.Vr = Vr
 
         # ---- H(k), mu -----------------------------------------------------
         self.Hk = np.stack([self.bloch_two_index(self.Hr, k) for k in range(self.nk)])

@@ -72,6 +72,7 @@ struct gwsig_ctx {
   long long launches = 0;
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
+  DevBuf oblk_ao, oblk_aux, unf_tmp;             // Eq. 28: O_block tables and the scratch T of the two-step block unfold
   DevBuf h_g, h_w, h_sig, h_vslot[2];           // device side of sigma_eval_host
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_freed[2] = {nullptr, nullptr};
@@ -198,6 +199,11 @@ int prepare_tables(gwsig_ctx* ctx) {
     if ((rc = upload(ctx, ctx->tgt_src, src))) return rc;
     if ((rc = upload(ctx, ctx->tgt_op, op))) return rc;
   }
+  if (P.mode == GWSIG_IBZ_BLOCK && P.general_gauge) {
+    int rc;
+    if ((rc = upload(ctx, ctx->oblk_ao, P.oblk_ao))) return rc;
+    if ((rc = upload(ctx, ctx->oblk_aux, P.oblk_aux))) return rc;
+  }
   // epilogue descriptors: one batch of ntau square matrices per (output k, block)
   std::vector<EpiDesc> ed;
   for (int i = 0; i < P.nk1; ++i) {
@@ -280,6 +286,34 @@ int run_stage(gwsig_ctx* ctx, int kind, const DevStage& d, const double2* A, con
   return GWSIG_OK;
 }
 
+// Eq. 28: X_blk^{k'}(tau) = O_block X_blk^{k_I}(tau) O_block^dagger for mesh points [k_first, k_first + k_count),
+// two launches of the grouped engine (step 1 into the scratch T, step 2 into dst).  aux: W with the auxiliary blocks.
+int run_block_unfold(gwsig_ctx* ctx, bool aux, int k_first, int k_count, const double2* src, double2* dst) {
+  const Plan& P = ctx->plan;
+  const long long elems = P.unfolded_elems(aux, k_first, k_count);
+  CU(ctx->unf_tmp.ensure(std::max<size_t>((size_t)elems * sizeof(double2), 16)));
+  const double2* O = (const double2*)(aux ? ctx->oblk_aux.p : ctx->oblk_ao.p);
+  for (int step = 1; step <= 2; ++step) {
+    StagePlan sp;
+    int rc = P.build_unfold(aux, k_first, k_count, step, sp);
+    if (rc) return fail(ctx, rc, "internal: build_unfold failed");
+    DevStage d;
+    d.nprob = (int)sp.prob.size();
+    d.ntiles = sp.ntiles;
+    if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
+    if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
+    if ((rc = upload(ctx, d.bucket, sp.bucket))) return rc;
+    rc = run_stage(ctx, aux ? GWSIG_KIND_UNFOLD_W : GWSIG_KIND_UNFOLD_G, d, step == 1 ? src : (const double2*)ctx->unf_tmp.p, O,
+                   step == 1 ? (double2*)ctx->unf_tmp.p : dst, 0);
+    // the descriptor tables are read by the kernel just enqueued: free them only after it has run
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    d.prob.release(); d.seg.release(); d.bucket.release();
+    if (rc) return rc;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "block unfold");
+  }
+  return GWSIG_OK;
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -297,7 +331,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -351,9 +385,6 @@ int gwsig_set_blocks(gwsig_ctx* ctx, const int* nblk_ao, const int* ao_block_off
                      const int* aux_block_off, const double* U_ao, const double* U_aux) {
   if (!ctx) return GWSIG_ERR_ARG;
   invalidate(ctx);
-  if (U_ao || U_aux)
-    return fail(ctx, GWSIG_ERR_ARG, "set_blocks: explicit U (general gauge, Eq. 28 unfold) is not available yet; pass NULL "
-                                    "and use the gauge U^{k'} = O^{k_I}(alpha) U^{k_I}");
   int rc = ctx->plan.set_blocks(nblk_ao, ao_block_off, nblk_aux, aux_block_off, U_ao, U_aux);
   return rc ? fail(ctx, rc, ctx->plan.err) : rc;
 }
@@ -472,7 +503,8 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
   const Plan& P = ctx->plan;
   if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
   StagePlan sp;
-  int rc = P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
+  int rc = stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
+                       : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_counts: bad range / stage");
   if (nproblems) *nproblems = (int64_t)sp.prob.size();
   if (nsegs) *nsegs = (int64_t)sp.seg.size();
@@ -485,7 +517,8 @@ int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, vo
   const Plan& P = ctx->plan;
   if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
   StagePlan sp;
-  int rc = P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
+  int rc = stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
+                       : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_get: bad range / stage");
   std::memcpy(problems_out, sp.prob.data(), sp.prob.size() * sizeof(gwsig_problem));
   std::memcpy(segs_out, sp.seg.data(), sp.seg.size() * sizeof(gwsig_seg));
@@ -530,6 +563,11 @@ int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSig
     if ((rc = toc(ctx))) return rc;
     ctx->launches++;
   }
+  if (P.mode == GWSIG_IBZ_BLOCK && P.general_gauge) {
+    // [a1] block basis, explicit gauge: G_blk(k') = O_block G_blk(k_I) O_block^dagger for every mesh point (Eq. 28)
+    CU(ctx->gbz.ensure(std::max<size_t>((size_t)P.gu_off[P.nk] * sizeof(double2), 16)));
+    if ((rc = run_block_unfold(ctx, false, 0, P.nk, ctx->dG, (double2*)ctx->gbz.p))) return rc;
+  }
   ctx->next_pair = 0;
   ctx->in_eval = true;
   return GWSIG_OK;
@@ -547,7 +585,8 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
   const int nk1 = P.nk1;
 
   const double2* Wsrc = P.mode == GWSIG_IBZ ? nullptr : ctx->dW;     // IBZ: the ring, filled per sub-batch below
-  const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
+  const bool blk_unfold = P.mode == GWSIG_IBZ_BLOCK && P.general_gauge;
+  const double2* Gsrc = (P.mode == GWSIG_IBZ || blk_unfold) ? (const double2*)ctx->gbz.p : ctx->dG;
 
   // sub-batches of pairs (whole q's where possible) and tau chunks sized to the scratch budget
   const double budget = (double)ctx->scratch_mib * 1048576.0 / (2.0 * sizeof(double2));   // elements of X (= of Y)
@@ -588,6 +627,13 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       CU(launch_unfold_sparse(up, nq, ctx->stream));
       if ((rc = toc(ctx))) return rc;
       ctx->launches++;
+      Wsrc = (const double2*)ctx->wring.p;
+    } else if (blk_unfold) {
+      // [a2] block basis, explicit gauge: W_blk(q) = O_block W_blk(q_I) O_block^dagger for the q of this sub-batch (Eq. 28 / 25)
+      const int nq = (int)((s1 - 1) / nk1) - q_sub + 1;
+      CU(ctx->wring.ensure(std::max<size_t>((size_t)P.unfolded_elems(true, q_sub, nq) * sizeof(double2), 16)));
+      int rc = run_block_unfold(ctx, true, q_sub, nq, ctx->dW, (double2*)ctx->wring.p);
+      if (rc) return rc;
       Wsrc = (const double2*)ctx->wring.p;
     }
     for (int t0 = 0; t0 < P.ntau; t0 += nt) {

@@ -216,7 +216,9 @@ int Plan::set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nbl
     const cplx* ux = reinterpret_cast<const cplx*>(U_aux_);
     U_ao.assign(ua, ua + (size_t)nk * nao * nao);
     U_aux.assign(ux, ux + (size_t)nk * naux * naux);
-  } else { U_ao.clear(); U_aux.clear(); }
+    if ((rc = compute_oblock(false))) return rc;
+    if ((rc = compute_oblock(true))) return rc;
+  } else { U_ao.clear(); U_aux.clear(); oblk_ao.clear(); oblk_aux.clear(); }
   have_blocks = true;
   have_triples = false;
   triple_ptr.clear(); triples.clear();
@@ -262,6 +264,8 @@ int Plan::finalize_layouts() {
   }
   g_elems = g_in_off.back();
   w_elems = w_in_off.back();
+  gu_off.assign(nk + 1, 0);
+  for (int k = 0; k < nk; ++k) gu_off[k + 1] = gu_off[k] + (blk ? sumsq(ao_off[k]) : (long long)nao * nao) * ntau;
   sig_off.assign(nk1 + 1, 0);
   for (int i = 0; i < nk1; ++i)
     sig_off[i + 1] = sig_off[i] + (blk ? sumsq(ao_off[out_list[i]]) : (long long)nao * nao) * ntau;
@@ -290,10 +294,8 @@ int Plan::finalize_layouts() {
 void Plan::g_source(int k2, long long& off, long long& tstride) const {
   if (mode == GWSIG_IBZ_BLOCK) {
     tstride = sumsq(ao_off[k2]);
-    if (general_gauge) {      // unfolded packed buffer over the whole mesh, mesh order
-      off = 0;
-      for (int k = 0; k < k2; ++k) off += sumsq(ao_off[k]) * ntau;
-    } else off = g_in_off[ir_index[ir_of[k2]]];          // S5 gauge: data of the representative
+    if (general_gauge) off = gu_off[k2];                  // unfolded packed buffer over the whole mesh, mesh order (Eq. 28)
+    else off = g_in_off[ir_index[ir_of[k2]]];            // S5 gauge: data of the representative
   } else {
     tstride = (long long)nao * nao;
     off = (long long)k2 * ntau * tstride;               // dG itself (FULL_BZ) or the unfolded buffer (IBZ)
@@ -538,6 +540,142 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
       while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
       out.bucket[bkt] = (int)pi;
     }
+  }
+  return GWSIG_OK;
+}
+
+// O_block = U^{k'}^dagger O^{k_I}(alpha^) U^{k_I} for alpha = op_of[k']  (Eq. 28), with
+// O^{k_I}(alpha^) = D(alpha) . diag(exp(-2 pi i k' . s_x))  (Eq. 3; column (x,m) carries the phase of its atom).
+// Must come out block diagonal in the supplied block map; only the diagonal blocks are kept.
+int Plan::compute_oblock(bool aux) {
+  const int n = aux ? naux : nao;
+  const std::vector<cplx>& U = aux ? U_aux : U_ao;
+  const std::vector<double>& D = aux ? D_aux : D_ao;
+  const std::vector<int>& atom = aux ? aux_atom : ao_atom;
+  const std::vector<std::vector<int>>& offs = aux ? aux_off : ao_off;
+  std::vector<cplx>& ob = aux ? oblk_aux : oblk_ao;
+  std::vector<long long>& oo = aux ? oblk_aux_off : oblk_ao_off;
+  oo.assign(nk + 1, 0);
+  for (int k = 0; k < nk; ++k) oo[k + 1] = oo[k] + sumsq(offs[k]);
+  ob.assign((size_t)oo[nk], cplx(0, 0));
+  std::vector<cplx> OU((size_t)n * n), R((size_t)n * n);
+  for (int kp = 0; kp < nk; ++kp) {
+    const int kI = ir_of[kp], g = op_of[kp];
+    int nn[3];
+    kcoords(kp, nn);
+    const cplx* UI = &U[(size_t)kI * n * n];
+    const cplx* UP = &U[(size_t)kp * n * n];
+    const double* Dg = &D[(size_t)g * n * n];
+    // OU = D diag(phase) U^{k_I}   (D is sparse: skip zeros)
+    std::fill(OU.begin(), OU.end(), cplx(0, 0));
+    for (int r = 0; r < n; ++r)
+      for (int m = 0; m < n; ++m) {
+        const double d = Dg[(size_t)r * n + m];
+        if (d == 0.0) continue;
+        const int* sx = &shift[((size_t)g * natom + atom[m]) * 3];
+        const double ph = -2.0 * M_PI * ((double)nn[0] * sx[0] / N[0] + (double)nn[1] * sx[1] / N[1] + (double)nn[2] * sx[2] / N[2]);
+        const cplx w = d * cplx(std::cos(ph), std::sin(ph));
+        for (int c = 0; c < n; ++c) OU[(size_t)r * n + c] += w * UI[(size_t)m * n + c];
+      }
+    // R = U^{k'}^dagger OU
+    std::fill(R.begin(), R.end(), cplx(0, 0));
+    for (int m = 0; m < n; ++m)
+      for (int r = 0; r < n; ++r) {
+        const cplx u = std::conj(UP[(size_t)m * n + r]);
+        if (u == cplx(0, 0)) continue;
+        for (int c = 0; c < n; ++c) R[(size_t)r * n + c] += u * OU[(size_t)m * n + c];
+      }
+    const std::vector<int>& off = offs[kp];
+    double in_blk = 0, off_blk = 0;
+    long long o = oo[kp];
+    for (size_t b = 0; b + 1 < off.size(); ++b) {
+      const int nb = off[b + 1] - off[b];
+      for (int r = 0; r < nb; ++r)
+        for (int c = 0; c < nb; ++c) ob[(size_t)o + (size_t)r * nb + c] = R[(size_t)(off[b] + r) * n + off[b] + c];
+      o += (long long)nb * nb;
+    }
+    std::vector<int> lab(n);
+    for (size_t b = 0; b + 1 < off.size(); ++b)
+      for (int i = off[b]; i < off[b + 1]; ++i) lab[i] = (int)b;
+    for (int r = 0; r < n; ++r)
+      for (int c = 0; c < n; ++c) {
+        const double a_ = std::abs(R[(size_t)r * n + c]);
+        if (lab[r] == lab[c]) in_blk = std::max(in_blk, a_); else off_blk = std::max(off_blk, a_);
+      }
+    if (off_blk > 1e-8 * std::max(in_blk, 1e-300)) {
+      err = std::string("set_blocks: O_block = U^dagger O U of mesh point ") + std::to_string(kp) + " is not block diagonal in the " +
+            (aux ? "auxiliary" : "orbital") + " block map (Eq. 28)";
+      return GWSIG_ERR_BLOCKS;
+    }
+  }
+  return GWSIG_OK;
+}
+
+long long Plan::unfolded_elems(bool aux, int k_first, int k_count) const {
+  long long s = 0;
+  for (int k = k_first; k < k_first + k_count; ++k) s += sumsq(aux ? aux_off[k] : ao_off[k]) * ntau;
+  return s;
+}
+
+int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& out) const {
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0;
+  if (!general_gauge || k_first < 0 || k_count < 1 || k_first + k_count > nk || step < 1 || step > 2) return GWSIG_ERR_ARG;
+  const std::vector<std::vector<int>>& offs = aux ? aux_off : ao_off;
+  const std::vector<long long>& in_off = aux ? w_in_off : g_in_off;
+  const std::vector<long long>& oo = aux ? oblk_aux_off : oblk_ao_off;
+  long long uoff = 0;                                   // offset of point k in T / the unfolded buffer
+  for (int k = k_first; k < k_first + k_count; ++k) {
+    const std::vector<int>& off = offs[k];
+    const long long ts = sumsq(off);                    // elements per tau
+    long long bo = 0;
+    for (size_t b = 0; b + 1 < off.size(); ++b) {
+      const int nb = off[b + 1] - off[b];
+      gwsig_seg S; std::memset(&S, 0, sizeof(S));
+      gwsig_problem P; std::memset(&P, 0, sizeof(P));
+      if (step == 1) {
+        // T[(tau, r), c] = sum_m X^{k_I}[(tau, r), m] conj(O[c, m])
+        S.a_off = in_off[ir_index[ir_of[k]]] + bo;
+        S.am = lvl2(nb, ts, nb); S.ak = lvl1(1);
+        S.b_off = oo[k] + bo;
+        S.bk = lvl1(1); S.bn = lvl1(nb);                 // B[m, c] = O[c, m]
+        S.K = nb;
+        P.M = ntau * nb; P.N = nb;
+        P.c_off = uoff + bo;
+        P.cm = lvl2(nb, ts, nb); P.cn = lvl1(1);
+        P.flags = GWSIG_FLAG_CONJ_B | GWSIG_FLAG_A_KMAJOR;
+      } else {
+        // X^{k'}[(tau), r, c] = sum_m O[r, m] T[(tau), m, c], lowered transposed: rows (tau, c), columns r
+        S.a_off = uoff + bo;
+        S.am = lvl2(nb, ts, 1); S.ak = lvl1(nb);         // A[(tau, c), m] = T[tau][m][c]
+        S.b_off = oo[k] + bo;
+        S.bk = lvl1(1); S.bn = lvl1(nb);                 // B[m, r] = O[r, m]
+        S.K = nb;
+        P.M = ntau * nb; P.N = nb;
+        P.c_off = uoff + bo;
+        P.cm = lvl2(nb, ts, 1); P.cn = lvl1(nb);         // C[(tau, c), r] = X[tau][r][c]
+        P.flags = 0;
+      }
+      P.nbatch = 1;
+      P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+      out.seg.push_back(S); out.prob.push_back(P);
+      bo += (long long)nb * nb;
+    }
+    uoff += ts * ntau;
+  }
+  long long tb = 0;
+  for (auto& P : out.prob) {
+    P.tiles_m = zg_tiles_m(P.M);
+    P.tiles_n = zg_tiles_n(P.N);
+    P.tile_begin = tb;
+    tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
+  }
+  out.ntiles = tb;
+  out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
+  size_t pi = 0;
+  for (size_t bkt = 0; bkt < out.bucket.size(); ++bkt) {
+    const long long t = (long long)bkt << ZG_BUCKET_SHIFT;
+    while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
+    out.bucket[bkt] = (int)pi;
   }
   return GWSIG_OK;
 }

@@ -45,8 +45,13 @@ struct Plan {
 
   // ---- blocks (IBZ_BLOCK) -------------------------------------------------------------------
   std::vector<std::vector<int>> ao_off, aux_off;     // per k: nblk+1 offsets (trivial {0,n} in dense modes)
-  std::vector<cplx> U_ao, U_aux;                     // optional general gauge
+  std::vector<cplx> U_ao, U_aux;                     // optional explicit gauge (set_blocks with U)
   bool general_gauge = false;
+  // O_block = U^{k'}^dagger O^{k_I}(alpha^) U^{k_I} (Eq. 28) for op_of[k'], packed diagonal blocks per mesh
+  // point (block b of point k at oblk_*_off[k] + blk_off(b), row-major); only in the explicit gauge
+  std::vector<cplx> oblk_ao, oblk_aux;
+  std::vector<long long> oblk_ao_off, oblk_aux_off;  // [nk + 1]
+  std::vector<long long> gu_off;                     // [nk + 1] unfolded packed G over the whole mesh (elements, all tau)
   std::vector<long long> triple_ptr;                 // [npairs+1]
   std::vector<int32_t> triples;                      // [3*nt]
 
@@ -99,6 +104,14 @@ struct Plan {
   // split_k > 1 cuts the segment list of every stage-3 problem into that many parts (separate problems that add
   // into the same Sigma block); 0 = choose so that the launch has enough tiles for `num_sms` SMs
   int build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out, int num_sms = 148) const;
+  // Eq. 28 unfold of packed diagonal blocks for mesh points [k_first, k_first + k_count), all tau, as two grouped GEMMs:
+  //   step 1  T(tau) = X^{k_I}(tau) O_block^dagger     (A = packed wedge input, B = O_block, C = scratch T)
+  //   step 2  X^{k'}(tau) = O_block T(tau)             (A = T, B = O_block, C = unfolded buffer)
+  // aux = false: G with the orbital blocks, true: W with the auxiliary blocks.  T and the unfolded buffer share one layout:
+  // point-major from k_first, [tau][packed blocks].
+  int build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& out) const;
+  long long unfolded_elems(bool aux, int k_first, int k_count) const;
+  int compute_oblock(bool aux);
   void flop_counts(double& full_equiv, double& executed) const;
 };
 

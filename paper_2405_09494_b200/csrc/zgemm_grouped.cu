@@ -60,16 +60,22 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar) {
 __device__ __forceinline__ void mbar_arrive_cp_async(unsigned bar) {   // fires when this thread's prior cp.async land
   asm volatile("cp.async.mbarrier.arrive.noinc.shared.b64 [%0];\n" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+  unsigned ok;
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared.b64 p, [%0], %1;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}\n" ::"r"(bar),
-      "r"(parity)
+      "mbarrier.try_wait.parity.shared.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}\n"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
       : "memory");
+  return ok != 0;
+}
+// a wait that cannot complete (a protocol bug) traps after ~2^26 polls instead of hanging the GPU until the job is killed
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned spins = 0;
+  while (!mbar_try_wait(bar, parity))
+    if (++spins > (1u << 26)) __trap();
 }
 
 // D(8x8) += A(8x4) * B(4x8), FP64 tensor core.  SASS: DMMA.8x8x4
@@ -438,12 +444,16 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
 //   sign of P2 in the epilogue.  At the end of a tile the MMA warps drop their accumulators into a shared staging
 //   buffer [3][128][33] and go straight on with the next tile; the epilogue warps combine the three planes, do the
 //   two-level C addressing and store (or red.add) with full-line global accesses in the orientation C is
-//   contiguous in.  Register budget per SM: 12 x 32 x 136 + 4 x 32 x 40 + 4 x 32 x 56 = 64512 <= 65536.
+//   contiguous in.  Register budget per CTA: 12 x 32 x 128 + 4 x 32 x 40 + 4 x 32 x 56 = 61440 = 640 x 96 at launch.
 // ------------------------------------------------------------------------------------------
 constexpr int kMmaWarps = 12;
 constexpr int kEpiWarps = 4;
-constexpr int kMmaRegs = 136, kLoaderRegs3 = 40, kEpiRegs = 56;
+constexpr int kMmaRegs = 128, kLoaderRegs3 = 40, kEpiRegs = 56;
 constexpr int kThreads3 = (kMmaWarps + kProducerWarps + kEpiWarps) * 32;
+constexpr int kLaunchRegs3 = 96;                       // what __launch_bounds__(640, 1) gives every thread: 65536 / 640 -> 96
+// setmaxnreg only moves registers INSIDE the CTA's launch-time allocation: an inc beyond it waits forever
+static_assert(32 * (kMmaWarps * kMmaRegs + kProducerWarps * kLoaderRegs3 + kEpiWarps * kEpiRegs) <= kThreads3 * kLaunchRegs3,
+              "setmaxnreg budget exceeds the launch-time register allocation of the CTA");
 constexpr int STG_LD = ZG_BN + 1;                      // odd pitch (doubles): conflict-free in both epilogue orientations
 constexpr int kTrec3 = kStages + 3;                    // loaders <= kStages tiles ahead of the MMA warps, epilogue one behind
 

@@ -15,8 +15,9 @@ class Configured:
     """a Gwsig context with lattice / symmetry (/ blocks) set, plus the host pre-step objects."""
 
     def __init__(self, lib: Gwsig, mode: int, a, mesh, nao, naux, ntau, beta, pos, ao_atom, aux_atom,
-                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7, out_points=None):
+                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7, out_points=None, scramble_gauge=None):
         self.lib, self.mode = lib, mode
+        self.general_gauge = scramble_gauge is not None and mode == IBZ_BLOCK
         self.nao, self.naux, self.ntau = nao, naux, ntau
         lib.set_lattice(a, mesh, nao, naux, ntau, beta)
         self.setup = None
@@ -39,7 +40,12 @@ class Configured:
         self.out_list = (np.arange(self.nk) if mode == FULL_BZ else self.ir_list) if out_points is None else np.asarray(out_points)
         if mode == IBZ_BLOCK:
             self.ao, self.aux = self.setup.adapt("ao"), self.setup.adapt("aux")
-            lib.set_blocks(self.ao.off, self.aux.off)
+            if scramble_gauge is None:
+                lib.set_blocks(self.ao.off, self.aux.off)                 # gauge S5: O_block = 1, no U needed
+            else:                                                         # general gauge: the library forms O_block (Eq. 28)
+                self.ao = self.setup.scramble(self.ao, scramble_gauge)
+                self.aux = self.setup.scramble(self.aux, scramble_gauge + 1)
+                lib.set_blocks(self.ao.off, self.aux.off, self.ao.U, self.aux.U)
 
     # ---- inputs -------------------------------------------------------------------------------
     def pack_GW(self, G_of, W_of):
@@ -101,8 +107,9 @@ class Configured:
         return out
 
 
-def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7, out_points=None) -> Configured:
+def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7, out_points=None, scramble_gauge=None) -> Configured:
     """convenience for the synthetic crystals of gwsig_synth (any object with the same fields)."""
     sg = cr.sg
     return Configured(lib, mode, cr.a, cr.mesh, cr.nao, cr.naux, cr.ntau, cr.beta, cr.pos, cr.ao_atom, cr.aux_atom,
-                      W=sg.W, w=sg.w, shift=sg.shift, P_ao=cr.P_ao, P_aux=cr.P_aux, seed=seed, out_points=out_points)
+                      W=sg.W, w=sg.w, shift=sg.shift, P_ao=cr.P_ao, P_aux=cr.P_aux, seed=seed, out_points=out_points,
+                      scramble_gauge=scramble_gauge)

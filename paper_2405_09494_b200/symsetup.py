@@ -148,6 +148,23 @@ class SymSetup:
                 off[k] = off[kI]
         return BlockBasis(U=U, off=off)
 
+    def scramble(self, basis: BlockBasis, seed: int) -> BlockBasis:
+        """an equally valid symmetry-adapted basis in a GENERAL gauge: U'^k = U^k . blockdiag(random unitaries), drawn
+        independently at EVERY mesh point (the adapted basis is only fixed up to a unitary inside each isotypic block,
+        PAPER.md:112-116).  Star members then no longer satisfy U^{k'} = O U^{k_I}, and O_block of Eq. 28
+         is a genuine block-diagonal unitary instead of the identity."""
+        U = np.empty_like(basis.U)
+        for k in range(self.nk):
+            rng = np.random.Generator(np.random.Philox(key=[seed, k]))
+            R = np.zeros(basis.U[k].shape, dtype=complex)
+            off = basis.off[k]
+            for b in range(len(off) - 1):
+                nb = off[b + 1] - off[b]
+                Q, _ = np.linalg.qr(rng.standard_normal((nb, nb)) + 1j * rng.standard_normal((nb, nb)))
+                R[off[b]:off[b + 1], off[b]:off[b + 1]] = Q
+            U[k] = basis.U[k] @ R
+        return BlockBasis(U=U, off=basis.off)
+
     # ---- Eq. 26-27: block-basis inputs, packed --------------------------------
     @staticmethod
     def pack_diag_blocks(X: np.ndarray, U: np.ndarray, off: np.ndarray, check: float = 1e-9):

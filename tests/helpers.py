@@ -139,6 +139,10 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
             O = rep_at_k(P[g], atom, cr.sg.shift[g], cr.kmesh.frac[k])
             return O @ X[ir_index[int(cfg.ir_of[k])]] @ O.conj().T
         Gsrc = np.stack([unfold(Gi, cr.P_ao, cr.ao_atom, k) for k in range(nk)]).ravel()
+    elif getattr(cfg, "general_gauge", False):
+        # Eq. 28: packed blocks of every mesh point through the two unfold launches (plan stages 11, 12) with the library's O_block
+        Oao, Oaux = block_O(cfg, inp, "ao"), block_O(cfg, inp, "aux")
+        Gsrc = unfold_blocks_numpy(lib, 11, 0, nk, G_flat, Oao, ntau)
     else:
         Gsrc = G_flat
     voff = [lib.pair_info(p)[3] for p in range(cfg.npairs)] + [V_flat.size]
@@ -148,6 +152,8 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
         q_first, q_last = p0 // cfg.nk1, (p0 + npp - 1) // cfg.nk1
         if cfg.mode == IBZ:
             Wsrc = np.stack([unfold(Wi, cr.P_aux, cr.aux_atom, q) for q in range(q_first, q_last + 1)]).ravel()
+        elif getattr(cfg, "general_gauge", False):
+            Wsrc = unfold_blocks_numpy(lib, 21, q_first, q_last - q_first + 1, W_flat, Oaux[q_first:q_last + 1], ntau)
         else:
             Wsrc = W_flat
         Vsub = V_flat[voff[p0]:voff[p0 + npp]]
@@ -163,3 +169,38 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
             run_stage_numpy(pr, sg, Y, Vsub, acc, t0)
         p0 += npp
     return -acc / nk
+
+
+def block_O(cfg, inp, kind):
+    """test-side O_block = U^{k'}^dagger O^{k_I}(alpha^) U^{k_I} (Eq. 28), packed diagonal blocks per mesh point
+    (list of flat arrays) -- what gwsig_set_blocks computes internally from U."""
+    cr = inp.cr
+    basis = cfg.ao if kind == "ao" else cfg.aux
+    P, atom = (cr.P_ao, cr.ao_atom) if kind == "ao" else (cr.P_aux, cr.aux_atom)
+    out = []
+    for k in range(cfg.nk):
+        g, kI = int(cfg.op_of[k]), int(cfg.ir_of[k])
+        O = rep_at_k(P[g], atom, cr.sg.shift[g], cr.kmesh.frac[k])
+        R = basis.U[k].conj().T @ O @ basis.U[kI]
+        off = basis.off[k]
+        out.append(np.concatenate([R[off[b]:off[b + 1], off[b]:off[b + 1]].ravel() for b in range(len(off) - 1)]))
+    return out
+
+
+def unfold_blocks_numpy(lib, stage0, k_first, k_count, X_flat, O_list, ntau):
+    """run the two unfold launches (stage0 = 11 for G, 21 for W) with the numpy interpreter; O_list: packed O_block of the
+    points k_first .. k_first + k_count - 1 (the library addresses O from mesh point 0: pad in front)."""
+    pr1, sg1, _ = lib.plan_get(k_first, k_count, ntau, stage0)
+    pr2, sg2, _ = lib.plan_get(k_first, k_count, ntau, stage0 + 1)
+    Oall = np.concatenate(O_list)
+    # b_off of the descriptors is relative to the whole-mesh O table: shift to this slice
+    shift = int(min(S["b_off"] for S in sg1))
+    Opad = np.concatenate([np.zeros(shift, complex), Oall])
+    n_out = 0
+    for P in pr1:
+        n_out = max(n_out, int(P["c_off"] + _idx(P["cm"], P["M"])[-1] + _idx(P["cn"], P["N"])[-1] + 1))
+    T = np.zeros(n_out, complex)
+    run_stage_numpy(pr1, sg1, X_flat, Opad, T, 0)
+    out = np.zeros(n_out, complex)
+    run_stage_numpy(pr2, sg2, T, Opad, out, 0)
+    return out

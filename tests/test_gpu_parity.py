@@ -185,6 +185,21 @@ def test_cfg3_shaped_small_mesh_full_oracle():
     _check(cfg, inp, run_gpu(cfg, G, W, V))
 
 
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite"])
+def test_general_gauge_eq28(name):
+    """explicit U in a scrambled gauge (independent random unitary inside every irrep block at EVERY mesh point): the
+    library forms O_block = U^{k'}^dagger O U^{k_I} and unfolds the packed G and W blocks with it (Eq. 28)."""
+    B = _B()
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    inp = get_inputs(name)
+    lib = B.Gwsig(device=0)
+    cfg = configure_from_crystal(lib, inp.cr, 2, scramble_gauge=5)
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    V = cfg.pack_V(inp.V2_rows)
+    _check(cfg, inp, run_gpu(cfg, G, W, V))
+    _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=1, engine=2))
+
+
 def test_output_point_subset_matches_full_run():
     B, inp, cfg, G, W, V = _setup("toy_diamond", 2)
     full = cfg.unpack_sigma(run_gpu(cfg, G, W, V))

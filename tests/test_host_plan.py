@@ -165,3 +165,27 @@ def test_stage3_split_k_parts_tile_the_segments():
     for a in range(len(cfg.out_list)):
         for t in range(inp.ntau):
             assert rel_err(got[a][t], ref[a, t]) < 1e-12
+
+
+@pytest.mark.parametrize("name", ["toy_diamond", "toy_wurtzite"])
+def test_general_gauge_eq28_host_plan(name):
+    """explicit U in a scrambled gauge (a different random unitary inside every block at EVERY mesh point): the library
+    forms O_block = U^{k'}^dagger O U^{k_I} (Eq. 28) and its unfold + contraction descriptors, run by the numpy
+    interpreter, reproduce the oracle; a U that mixes blocks is refused."""
+    inp = make_inputs(name)
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ_BLOCK, scramble_gauge=5)
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    V = cfg.pack_V(inp.V2_rows)
+    sig = run_plan_numpy(cfg, inp, G, W, V, push_pairs=cfg.nk1 * 3)
+    got = fold_to_orbital(cfg, inp, cfg.unpack_sigma(sig))
+    ref = oracle_sigma(inp, range(inp.nk))
+    assert max(rel_err(got[k][t], ref[k, t]) for k in range(inp.nk) for t in range(inp.ntau)) < 1e-11
+    # a basis that mixes two blocks at a star member (not the representative, whose O_block is U^dagger U = 1) is refused
+    k_bad = next(k for k in range(cfg.nk) if len(cfg.ao.off[k]) > 2 and cfg.ir_of[k] != k)
+    Ubad = cfg.ao.U.copy()
+    o = cfg.ao.off[k_bad]
+    Ubad[k_bad][:, [o[0], o[1]]] = (Ubad[k_bad][:, [o[0], o[1]]] @ np.array([[1, 1], [1, -1]])) / np.sqrt(2)
+    with pytest.raises(B.GwsigError) as e:
+        lib.set_blocks(cfg.ao.off, cfg.aux.off, Ubad, cfg.aux.U)
+    assert e.value.code == -3

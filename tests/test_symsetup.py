@@ -121,3 +121,35 @@ def test_executed_mac_ratio_is_in_the_papers_range():
                 for (p, a, i) in tr:
                     blk += sp[p] * s1[i] * s2[a] ** 2 + sp[p] * s2[a] * s1[i] ** 2
         assert lo < blk / dense < hi, (name, blk / dense)
+
+
+def test_device_blocker_matches_block_V2():
+    """the batched (torch) Eq. 27 transform + triple detection + packing of presetup_device agrees with the per-pair numpy
+    pre-step symsetup.block_V2 on every pair of a toy crystal (run on the CPU here, on the GPU in bench.py)."""
+    import torch
+    from paper_2405_09494_b200 import binding as B
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    from paper_2405_09494_b200.presetup_device import DeviceBlocker
+    inp = make_inputs("toy_diamond4")
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ_BLOCK)
+    blk = DeviceBlocker(cfg, torch, torch.device("cpu"))
+    pairs = list(range(0, cfg.npairs, 7))[:40]
+    info = [lib.pair_info(p, with_layout=False) for p in pairs]
+    k1s, k2s, qs = [i[0] for i in info], [i[1] for i in info], [i[2] for i in info]
+    V = np.stack([inp.V2_rows(k1, [k2])[0] for k1, k2 in zip(k1s, k2s)])
+    T = blk.transform(torch.from_numpy(V), qs, k2s, k1s)
+    vmax = float(np.abs(V).max())
+    mx = blk.block_maxabs(T, qs, k2s, k1s)
+    trip = blk.triples_from_maxabs(mx, qs, k2s, k1s, 1e-9, vmax)
+    tabs = blk.pack_tables(trip, qs, k2s, k1s)
+    size = tabs[3]
+    off = np.concatenate([[0], np.cumsum(size)])
+    dst = torch.zeros(int(off[-1]), dtype=torch.complex128)
+    blk.pack(T, qs, k2s, k1s, tabs, dst, off[:-1])
+    for r, (k1, k2) in enumerate(zip(k1s, k2s)):
+        t_ref, packed_ref = cfg.setup.block_V2(V[r], k1, k2, cfg.ao, cfg.aux, thresh=1e-9, vmax=vmax)
+        assert np.array_equal(t_ref, trip[r])
+        got = dst[off[r]:off[r + 1]].numpy()
+        assert got.shape == packed_ref.shape
+        assert np.abs(got - packed_ref).max() <= 1e-13 * vmax
