@@ -196,3 +196,64 @@ def test_sigma_covariance_hermiticity_and_block_zeros(name):
 
 def test_flop_model():
     assert flops_per_output(8, 8, 32) == 8 * 8 * (2 * 32 * 512 + 1024 * 64)
+
+
+# ---- Hartree-Fock exchange, Eq. 21c --------------------------------------------------
+def test_exchange_brute_vs_ref_and_scalar_closed_form():
+    from oracle.exchange_oracle import exchange_brute, exchange_ref
+    inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=4, ntau=2, beta=3.0, nocc=1, seed=8)
+    rng = np.random.default_rng(3)
+    gamma = rng.standard_normal((inp.nk, 3, 3)) + 1j * rng.standard_normal((inp.nk, 3, 3))
+    # unrelated partners: the oracle must not assume V^{k'k} = conj-transpose of V^{kk'}
+    Vb = {(a, b): rng.standard_normal((4, 3, 3)) + 1j * rng.standard_normal((4, 3, 3)) for a in range(inp.nk) for b in range(inp.nk)}
+    Va = {(a, b): rng.standard_normal((4, 3, 3)) + 1j * rng.standard_normal((4, 3, 3)) for a in range(inp.nk) for b in range(inp.nk)}
+    calls = {"n": 0}
+
+    def V_pair(a, b):
+        # exchange_* ask for V^{k k'} first, V^{k' k} second
+        calls["n"] += 1
+        return Va[(a, b)] if calls["n"] % 2 == 1 else Vb[(a, b)]
+    ks = [0, 3]
+    brute = exchange_brute(inp.nk, gamma, V_pair, ks)
+    ref = exchange_ref(inp.nk, lambda k: gamma[k], V_pair, ks)
+    assert np.abs(brute - ref).max() < 1e-13 * np.abs(ref).max()
+    # independent einsum statement of Eq. 21c
+    for a, k in enumerate(ks):
+        want = -sum(np.einsum("Qia,ab,Qbj->ij", Va[(k, kp)], gamma[kp], Vb[(kp, k)]) for kp in range(inp.nk)) / inp.nk
+        assert np.abs(ref[a] - want).max() < 1e-13 * np.abs(want).max()
+    # scalar closed form: nao = naux = 1, k-independent v and gamma  =>  K = -|v|^2 gamma  (sign and 1/Nk)
+    v, g = 0.7 - 0.4j, 0.3 + 0.1j
+    K = exchange_ref(5, lambda k: np.array([[g]]), lambda a, b: np.array([[[v]]]) if a <= b else np.array([[[np.conj(v)]]]), [2])
+    # pairs (k,k') with k<k' contribute v*conj(v), k>k' conj(v)*v, k=k' v*v: write the expected sum out
+    want = -(2 * abs(v) ** 2 + 2 * abs(v) ** 2 + v * v) * g / 5
+    assert abs(K[0, 0, 0] - want) < 1e-15
+
+
+def test_exchange_is_eq16_with_delta_W_and_gamma():
+    """the paper's own relation: K^k (Eq. 21c) is Sigma^k (Eq. 16) with W -> delta_{QQ'} and G(k - q, tau) -> gamma^{k - q};
+    sigma_ref is pinned on its own above."""
+    from oracle.exchange_oracle import exchange_ref
+    from oracle.sigma_oracle import sigma_ref
+    inp = make_inputs("cfg1", mesh=(3, 2, 1), nao=3, naux=4, ntau=2, beta=3.0, nocc=1, seed=5)
+    rng = np.random.default_rng(11)
+    gamma = rng.standard_normal((inp.nk, 3, 3)) + 1j * rng.standard_normal((inp.nk, 3, 3))
+    ks = list(range(inp.nk))
+    K = exchange_ref(inp.nk, lambda k: gamma[k], inp.V_pair, ks)
+    S = sigma_ref(inp.nk, inp.kmesh.sub, lambda k: gamma[k][None], lambda q: np.eye(4, dtype=complex)[None], inp.V_pair, ks)
+    assert np.abs(K - S[:, 0]).max() < 1e-13 * np.abs(K).max()
+
+
+def test_exchange_gauge_covariance_and_hermiticity():
+    from oracle.exchange_oracle import exchange_ref
+    inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=4, ntau=2, beta=3.0, nocc=1, seed=6)
+    G = inp.G_full()
+    gamma = -G[:, -1]                                           # gamma^k = G^k(0^-) = -G^k(beta), Hermitian (PAPER.md:194)
+    ks = list(range(inp.nk))
+    K = exchange_ref(inp.nk, lambda k: gamma[k], inp.V_pair, ks)
+    assert np.abs(K - K.conj().transpose(0, 2, 1)).max() < 1e-13 * np.abs(K).max()       # V^{k'k} = V^{kk'}^dagger, gamma Hermitian
+    rng = np.random.default_rng(2)
+    T = [np.linalg.qr(rng.standard_normal((3, 3)) + 1j * rng.standard_normal((3, 3)))[0] for _ in range(inp.nk)]
+    K2 = exchange_ref(inp.nk, lambda k: T[k] @ gamma[k] @ T[k].conj().T,
+                      lambda a, b: np.einsum("ip,Qpq,jq->Qij", T[a], inp.V_pair(a, b), T[b].conj()), ks)
+    for k in ks:
+        assert np.abs(K2[k] - T[k] @ K[k] @ T[k].conj().T).max() < 1e-13 * np.abs(K).max()
