@@ -163,6 +163,16 @@ int gwsig_sigma_abort(gwsig_ctx* ctx);
 int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, const void* hW, void* hSigma,
                           void* stream);
 
+/* ---- N2: Hartree-Fock exchange -------------------------------------------------
+ * K^k_ij = -(1/Nk) sum_{k'} sum_{ab} sum_Q V^{k k'}_{ia}(Q) gamma^{k'}_{ab} V^{k' k}_{bj}(Q)       (Eq. 21c)
+ * is Eq. 16 with W -> delta_{QQ'} and G(k - q, tau) -> the density matrix gamma^{k'}: the same pair list,
+ * the same V2 operand, stage 1 (X = V gamma) feeding stage 3 (K += X V) directly, stage 2 skipped.  dGamma has the layout
+ * of G with the context's ntau slices treated as independent density matrices (set ntau = 1 in set_lattice for one
+ * gamma per k); dK has the layout of Sigma.  exchange_begin is followed by sigma_push_pairs ... sigma_end (or
+ * sigma_abort) exactly as sigma_begin is; exchange_eval = begin + one push of all pairs + end.                       */
+int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream);
+int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream);
+
 /* ---- options and accounting ------------------------------------------------------------------ */
 /* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
  * default 8192), "tau_chunk" (0 = from the budget), "v_ring_mib" (size of one slot of the

@@ -64,6 +64,7 @@ struct gwsig_ctx {
   int tau_chunk = 0;
   // evaluation state
   bool in_eval = false;
+  bool exchange = false;        // evaluation opened by exchange_begin: no W, stage 2 skipped (Eq. 21c)
   const double2* dG = nullptr;
   const double2* dW = nullptr;
   double2* dSigma = nullptr;
@@ -532,7 +533,7 @@ int gwsig_sigma_begin(gwsig_ctx* ctx, const void* dG, const void* dW, void* dSig
   if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: call set_symmetry first");
   if (P.mode == GWSIG_IBZ_BLOCK && (!P.have_blocks || !P.have_triples))
     return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: IBZ_BLOCK mode needs set_blocks and set_triples");
-  if (!dG || !dW || !dSigma) return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: NULL device pointer");
+  if (!dG || (!dW && !ctx->exchange) || !dSigma) return fail(ctx, GWSIG_ERR_ARG, "sigma_begin: NULL device pointer");
   int rc = ensure_cuda(ctx);
   if (rc) return rc;
   CU(cudaSetDevice(ctx->device));
@@ -607,10 +608,12 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
     const int nt = (P.ntau + nchunks - 1) / nchunks;
     const size_t xbytes = (size_t)std::max(per_tau * nt, 1.0) * sizeof(double2);
     CU(ctx->xbuf.ensure(xbytes));
-    CU(ctx->ybuf.ensure(xbytes));
+    if (!ctx->exchange) CU(ctx->ybuf.ensure(xbytes));
     const double2* Vsub = Vbase + (P.v_off[s0] - P.v_off[p0]);
     const int q_sub = (int)(s0 / nk1);                 // first q of this sub-batch = first q held by the W ring
-    if (P.mode == GWSIG_IBZ) {
+    if (ctx->exchange) {
+      // Eq. 21c: W -> delta, nothing to unfold
+    } else if (P.mode == GWSIG_IBZ) {
       // [a2] unfold W for the q of this sub-batch only (Eq. 25; Algorithm 4 line 6): the ring holds a few
       // q, never the whole zone (100 GB at cfg5)
       const int nq = (int)((s1 - 1) / nk1) - q_sub + 1;
@@ -642,8 +645,10 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       int rc = get_dev_plan(ctx, s0, ns, ntc, q_sub, &dp);
       if (rc) return rc;
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], Gsrc, Vsub, (double2*)ctx->xbuf.p, t0))) return rc;                     // [a3]
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->ybuf.p, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
+      if (!ctx->exchange &&
+          (rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
+      const double2* Ysrc = (const double2*)(ctx->exchange ? ctx->xbuf.p : ctx->ybuf.p);     // Eq. 21c: Y = X (W = delta)
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], Ysrc, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
     }
     s0 = s1;
   }
@@ -670,6 +675,7 @@ int gwsig_sigma_end(gwsig_ctx* ctx) {
   if ((rc = toc(ctx))) return rc;
   ctx->launches++;
   ctx->in_eval = false;
+  ctx->exchange = false;
   return GWSIG_OK;
 }
 
@@ -685,7 +691,26 @@ int gwsig_sigma_abort(gwsig_ctx* ctx) {
   if (!ctx) return GWSIG_ERR_ARG;
   if (!ctx->in_eval) return fail(ctx, GWSIG_ERR_ORDER, "sigma_abort: no evaluation is open");
   ctx->in_eval = false;
+  ctx->exchange = false;
   return GWSIG_OK;
+}
+
+/* ---- N2: Hartree-Fock exchange K^k (Eq. 21c) = Eq. 16 with W -> delta_{QQ'} and G(tau) -> gamma --------- */
+int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  if (ctx->in_eval) return fail(ctx, GWSIG_ERR_ORDER, "exchange_begin: an evaluation is already open");
+  ctx->exchange = true;
+  int rc = gwsig_sigma_begin(ctx, dGamma, nullptr, dK, stream);
+  if (rc) ctx->exchange = false;
+  return rc;
+}
+
+int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream) {
+  int rc = gwsig_exchange_begin(ctx, dGamma, dK, stream);
+  if (rc) return rc;
+  rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
+  if (rc) { ctx->in_eval = false; ctx->exchange = false; return rc; }
+  return gwsig_sigma_end(ctx);
 }
 
 int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, const void* hW, void* hSigma, void* stream) {

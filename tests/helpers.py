@@ -119,7 +119,26 @@ def run_stage_numpy(prob, seg, A, B, C, t0):
                 C[ci] = acc
 
 
-def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
+def oracle_exchange(inp, gamma_of, ks):
+    """oracle/exchange_oracle.exchange_ref with independently generated V^{k k'} (V1_rows) and V^{k' k} (V2_rows)."""
+    from oracle.exchange_oracle import exchange_ref
+    out = []
+    for k in ks:
+        k = int(k)
+        k2s = list(range(inp.nk))
+        rows1, rows2 = inp.V1_rows(k, k2s), inp.V2_rows(k, k2s)
+        diag = [0]
+
+        def V_pair(a, b, k=k, rows1=rows1, rows2=rows2, diag=diag):
+            if a == k and b == k:
+                diag[0] ^= 1
+                return rows1[k] if diag[0] else rows2[k]
+            return rows1[b] if a == k else rows2[a]
+        out.append(exchange_ref(inp.nk, gamma_of, V_pair, [k])[0])
+    return np.stack(out)
+
+
+def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None, exchange=False):
     """emulate gwsig_sigma_eval's orchestration with the descriptors of gwsig_plan_get()."""
     lib = cfg.lib
     ntau, nao, naux, nk = cfg.ntau, cfg.nao, cfg.naux, cfg.nk
@@ -131,7 +150,7 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
     if cfg.mode == IBZ:
         cr = inp.cr
         Gi = G_flat.reshape(len(cfg.ir_list), ntau, nao, nao)
-        Wi = W_flat.reshape(len(cfg.ir_list), ntau, naux, naux)
+        Wi = None if exchange else W_flat.reshape(len(cfg.ir_list), ntau, naux, naux)
         ir_index = {int(k): i for i, k in enumerate(cfg.ir_list)}
 
         def unfold(X, P, atom, k):
@@ -150,7 +169,9 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
     while p0 < cfg.npairs:
         npp = min(push_pairs, cfg.npairs - p0)
         q_first, q_last = p0 // cfg.nk1, (p0 + npp - 1) // cfg.nk1
-        if cfg.mode == IBZ:
+        if exchange:
+            Wsrc = None
+        elif cfg.mode == IBZ:
             Wsrc = np.stack([unfold(Wi, cr.P_aux, cr.aux_atom, q) for q in range(q_first, q_last + 1)]).ravel()
         elif getattr(cfg, "general_gauge", False):
             Wsrc = unfold_blocks_numpy(lib, 21, q_first, q_last - q_first + 1, W_flat, Oaux[q_first:q_last + 1], ntau)
@@ -163,8 +184,11 @@ def run_plan_numpy(cfg, inp, G_flat, W_flat, V_flat, push_pairs=None, nt=None):
             Y = np.zeros(Vsub.size * ntc, complex)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 1)
             run_stage_numpy(pr, sg, Gsrc, Vsub, X, t0)
-            pr, sg, _ = lib.plan_get(p0, npp, ntc, 2)
-            run_stage_numpy(pr, sg, X, Wsrc, Y, t0)
+            if exchange:                       # Eq. 21c: W -> delta, stage 2 skipped, stage 3 reads X
+                Y = X
+            else:
+                pr, sg, _ = lib.plan_get(p0, npp, ntc, 2)
+                run_stage_numpy(pr, sg, X, Wsrc, Y, t0)
             pr, sg, _ = lib.plan_get(p0, npp, ntc, 3)
             run_stage_numpy(pr, sg, Y, Vsub, acc, t0)
         p0 += npp

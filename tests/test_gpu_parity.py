@@ -4,7 +4,7 @@ FP64, after folding the result back to the orbital basis."""
 import numpy as np
 import pytest
 
-from tests.helpers import fold_to_orbital, get_inputs, oracle_sigma, rel_err
+from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_sigma, rel_err
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -198,6 +198,33 @@ def test_general_gauge_eq28(name):
     V = cfg.pack_V(inp.V2_rows)
     _check(cfg, inp, run_gpu(cfg, G, W, V))
     _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=1, engine=2))
+
+
+@pytest.mark.parametrize("name,mode", [("toy_diamond4", 2), ("toy_wurtzite", 1), ("cfg2", 2)])
+def test_exchange_eq21c(name, mode):
+    """N2: K^k = -(1/Nk) sum_{k'} V^{kk'} gamma^{k'} V^{k'k} (Eq. 21c) through gwsig_exchange_eval (stage 1 feeding
+    stage 3, no W) against oracle/exchange_oracle.py, gamma^k = G^k(0^-) = -G^k(beta), one slice (ntau = 1)."""
+    B = _B()
+    torch = _torch()
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    import copy
+    inp = get_inputs(name)
+    cr1 = copy.copy(inp.cr)
+    cr1.ntau = 1                                                   # the context sees one "tau" slice: the density matrix
+    lib = B.Gwsig(device=0)
+    cfg = configure_from_crystal(lib, cr1, mode)
+    gam = lambda k: -inp.G_k(int(k))[-1]
+    G, _ = cfg.pack_GW(lambda k: gam(k)[None], lambda q: np.zeros((1, inp.naux, inp.naux), complex))
+    V = cfg.pack_V(inp.V2_rows)
+    dG, dV = torch.from_numpy(G).cuda(), torch.from_numpy(V).cuda()
+    dK = torch.full((lib.buffer_sizes()[2],), float("nan"), dtype=torch.complex128, device="cuda")
+    lib.exchange_eval(dG, dV, dK, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    got = fold_to_orbital(cfg, inp, cfg.unpack_sigma(dK.cpu().numpy()))
+    ks = list(range(inp.nk)) if inp.nk <= 64 else list(range(0, inp.nk, 5))
+    ref = oracle_exchange(inp, gam, ks)
+    worst = max(rel_err(got[k][0], ref[a]) for a, k in enumerate(ks))
+    assert worst <= TOL, worst
 
 
 def test_output_point_subset_matches_full_run():

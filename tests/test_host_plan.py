@@ -189,3 +189,22 @@ def test_general_gauge_eq28_host_plan(name):
     with pytest.raises(B.GwsigError) as e:
         lib.set_blocks(cfg.ao.off, cfg.aux.off, Ubad, cfg.aux.U)
     assert e.value.code == -3
+
+
+def test_exchange_plan_skips_stage_two():
+    """N2 (Eq. 21c): the exchange call runs stage 1 and feeds stage 3 directly; the same descriptors, interpreted in numpy with
+    Y = X, reproduce oracle/exchange_oracle.py in block mode."""
+    import copy
+    from tests.helpers import oracle_exchange
+    inp = make_inputs("toy_diamond")
+    cr1 = copy.copy(inp.cr)
+    cr1.ntau = 1
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, cr1, B.IBZ_BLOCK)
+    gam = lambda k: -inp.G_k(int(k))[-1]
+    G, _ = cfg.pack_GW(lambda k: gam(k)[None], lambda q: np.zeros((1, inp.naux, inp.naux), complex))
+    V = cfg.pack_V(inp.V2_rows)
+    K = run_plan_numpy(cfg, inp, G, None, V, exchange=True)
+    got = fold_to_orbital(cfg, inp, cfg.unpack_sigma(K))
+    ref = oracle_exchange(inp, gam, range(inp.nk))
+    assert max(rel_err(got[k][0], ref[k]) for k in range(inp.nk)) < 1e-11
