@@ -578,9 +578,21 @@ def main():
                 continue
             w2 = Workload(args.workload, MODES[mname], B, pack, inp=wl.inp, nq_subset=nq, torch=torch, dev=dev, device_index=local)
             w2.lib.set_option("engine", args.engine)
-            tt, _, _, _ = run_steps(w2, torch, dev, 1, 1, timing=False)
+            tt, k2, _, _ = run_steps(w2, torch, dev, 1, 1, timing=(mname == "ibz"))
             scale = w2.cfg.nk / w2.nq
             modes[mname] = {"ms": tt[0] * 1e3 * scale, "gflop_executed": w2.executed / 1e9}
+            if mname == "ibz":
+                # the HBM-bound helper kernels of the IBZ mode (steps a1, a2): algorithmic bytes = unfolded output written once
+                # + the wedge source read once, against the measured copy bandwidth (MEASURED_PEAKS.json hbm_gbs)
+                c2 = w2.cfg
+                nik = len(c2.ir_list)
+                bg = 16.0 * c2.ntau * c2.nao ** 2 * (c2.nk + nik)
+                bw = 16.0 * c2.ntau * c2.naux ** 2 * (w2.nq + min(nik, w2.nq))
+                ug, uw = k2["unfold_G"][0] * 1e-3, k2["unfold_W"][0] * 1e-3
+                hbm = measured_hbm_gbs()
+                modes[mname]["unfold"] = {"G_ms": ug * 1e3, "W_ms": uw * 1e3, "G_gbs": bg / max(ug, 1e-12) / 1e9, "W_gbs": bw / max(uw, 1e-12) / 1e9,
+                                          "hbm_peak_gbs": hbm, "W_frac_of_measured_hbm": bw / max(uw, 1e-12) / 1e9 / hbm,
+                                          "share_of_step": (ug + uw) / tt[0]}
             if scale != 1:
                 modes[mname]["note"] = f"timed on the first {w2.nq} of {w2.cfg.nk} q slices (all k1, all tau; every slice costs the same), scaled x{scale:g}"
             del w2
@@ -593,6 +605,13 @@ def main():
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def measured_hbm_gbs():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        return 6650.0            # the profiling guide's fallback
 
 
 def describe(name):

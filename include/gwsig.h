@@ -177,7 +177,10 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
 /* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
  * default 8192), "tau_chunk" (0 = from the budget), "v_ring_mib" (size of one slot of the
  * V ring of sigma_eval_host, default 1024), "timing" (0/1: record a CUDA event pair around
- * every kernel launch on the launching stream, read back with gwsig_kernel_times)                  */
+ * every kernel launch on the launching stream, read back with gwsig_kernel_times),
+ * "deterministic" (0/1, default 0): 1 = the split-K parts of stage 3 write private partial tiles that are summed into
+ * Sigma in a fixed order by a reduction kernel instead of FP64 atomics in scheduler order: results are then bit-identical
+ * from run to run (same device, same options); costs one extra pass over the partial tiles                         */
 int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value);
 /* real flops (8 per complex multiply-add) of one evaluation: the full-BZ dense equivalent
  * Nk^2 ntau 8(2A+B) and what the current mode's plan actually asks for.

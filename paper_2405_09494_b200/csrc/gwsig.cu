@@ -42,9 +42,9 @@ struct DevBuf {
 };
 
 struct DevStage {
-  DevBuf prob, seg, bucket;
-  int nprob = 0;
-  long long ntiles = 0;
+  DevBuf prob, seg, bucket, red;
+  int nprob = 0, nred = 0;
+  long long ntiles = 0, partial_elems = 0;
 };
 struct DevPlan { DevStage st[3]; };
 
@@ -73,7 +73,8 @@ struct gwsig_ctx {
   long long launches = 0;
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
-  DevBuf oblk_ao, oblk_aux, unf_tmp;             // Eq. 28: O_block tables and the scratch T of the two-step block unfold
+  DevBuf oblk_ao, oblk_aux, unf_tmp, partial;    // partial: split-K partial tiles of deterministic stage 3
+  DevBuf __unused_;             // Eq. 28: O_block tables and the scratch T of the two-step block unfold
   DevBuf h_g, h_w, h_sig, h_vslot[2];           // device side of sigma_eval_host
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_freed[2] = {nullptr, nullptr};
@@ -239,6 +240,9 @@ int get_dev_plan(gwsig_ctx* ctx, long long p0, long long np, int nt, int q_first
     if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
     if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
     if ((rc = upload(ctx, d.bucket, sp.bucket))) return rc;
+    d.nred = (int)sp.red.size();
+    d.partial_elems = sp.partial_elems;
+    if (d.nred && (rc = upload(ctx, d.red, sp.red))) return rc;
   }
   *out = dp.get();
   ctx->plan_cache[key] = std::move(dp);
@@ -332,7 +336,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -344,7 +348,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     for (auto& kv : ctx->plan_cache)
-      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); }
+      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
   }
   delete ctx;
   return GWSIG_OK;
@@ -355,7 +359,7 @@ const char* gwsig_last_error(const gwsig_ctx* ctx) { return ctx ? ctx->err.c_str
 static void invalidate(gwsig_ctx* ctx) {
   ctx->tables_ready = false;
   for (auto& kv : ctx->plan_cache)
-    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); }
+    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
   ctx->plan_cache.clear();
   ctx->in_eval = false;
 }
@@ -461,6 +465,7 @@ int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
   else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
   else if (k == "v_ring_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: v_ring_mib < 1"); ctx->v_ring_mib = value; }
   else if (k == "timing") ctx->timing = value != 0;
+  else if (k == "deterministic") { invalidate(ctx); ctx->plan.deterministic = value != 0; }
   else if (k == "tau_chunk") { if (value < 0) return fail(ctx, GWSIG_ERR_ARG, "set_option: tau_chunk < 0"); ctx->tau_chunk = (int)value; }
   else return fail(ctx, GWSIG_ERR_ARG, "set_option: unknown key " + k);
   return GWSIG_OK;
@@ -648,7 +653,14 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
       if (!ctx->exchange &&
           (rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->xbuf.p, Wsrc, (double2*)ctx->ybuf.p, t0))) return rc;  // [a4]
       const double2* Ysrc = (const double2*)(ctx->exchange ? ctx->xbuf.p : ctx->ybuf.p);     // Eq. 21c: Y = X (W = delta)
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], Ysrc, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
+      if (dp->st[2].nred) {
+        // deterministic accumulation: parts write private tiles, then one ordered reduction into the accumulator
+        CU(ctx->partial.ensure(std::max<size_t>((size_t)dp->st[2].partial_elems * sizeof(double2), 16)));
+        if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], Ysrc, Vsub, (double2*)ctx->partial.p, t0))) return rc;
+        CU(launch_reduce_parts((const RedGroupDev*)dp->st[2].red.p, dp->st[2].nred, (const double2*)ctx->partial.p, (double2*)ctx->sigacc.p, t0,
+                               ctx->stream));
+        ctx->launches++;
+      } else if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], Ysrc, Vsub, (double2*)ctx->sigacc.p, t0))) return rc; // [a5]
     }
     s0 = s1;
   }

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
+
 #include "kernels_aux.cuh"
 
 namespace {
@@ -62,6 +64,24 @@ __global__ void __launch_bounds__(256) epilogue_kernel(EpilogueParams p) {
       v.y = 0.5 * (v.y - w.y);
     }
     p.out[base + ij] = make_double2(p.scale * v.x, p.scale * v.y);
+  }
+}
+
+// deterministic stage 3: one thread per element of a Sigma block, the block's split-K partial tiles added in part order
+__global__ void __launch_bounds__(256) reduce_parts_kernel(const RedGroupDev* groups, const double2* partial, double2* acc, int t0) {
+  const RedGroupDev g = groups[blockIdx.y];
+  const long long total = (long long)g.M * g.ni;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const double2* src = partial + g.part_off + e;
+    double sr = 0.0, si = 0.0;
+    for (int p = 0; p < g.nparts; ++p) {
+      const double2 v = src[(long long)p * total];
+      sr += v.x; si += v.y;
+    }
+    const int row = (int)(e / g.ni), j = (int)(e - (long long)row * g.ni);      // row = (tau, i)
+    const int tau = row / g.ni, i = row - tau * g.ni;
+    double2* dst = acc + g.c_off + (long long)(t0 + tau) * g.sts + (long long)i * g.ni + j;
+    dst->x += sr; dst->y += si;
   }
 }
 
@@ -132,6 +152,15 @@ cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_
   if (ntarget <= 0) return cudaSuccess;
   dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n * p.n + 255) / 256));
   unfold_sparse_kernel<<<grid, 256, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream) {
+  if (ngroups <= 0) return cudaSuccess;
+  for (int g0 = 0; g0 < ngroups; g0 += 65535) {
+    dim3 grid(8, (unsigned)std::min(65535, ngroups - g0));
+    reduce_parts_kernel<<<grid, 256, 0, stream>>>(groups + g0, partial, acc, t0);
+  }
   return cudaGetLastError();
 }
 

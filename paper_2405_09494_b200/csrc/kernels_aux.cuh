@@ -29,6 +29,12 @@ struct EpilogueParams {
   int hermitize;
 };
 
+struct RedGroupDev {      // = gwsig::RedGroup (plan.hpp)
+  long long c_off, sts, part_off;
+  int ni, M, nparts, pad_;
+};
+// acc[block] += sum over the block's partial tiles IN PART ORDER (deterministic stage 3)
+cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream);
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream);
 cudaError_t launch_epilogue(const EpilogueParams& p, int ndesc, int num_sms, cudaStream_t stream);
 cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long iters, double* sink, cudaStream_t stream,

@@ -319,7 +319,7 @@ static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo;
 static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
 
 int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out, int num_sms) const {
-  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0;
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
   if (p0 < 0 || np < 1 || p0 + np > npairs || nt < 1 || nt > ntau || stage < 1 || stage > 3) return GWSIG_ERR_ARG;
   if (v_off.empty()) return GWSIG_ERR_ARG;
 
@@ -499,9 +499,17 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
       parts = std::min<long long>(parts, (long long)x.segs.size());
       size_t s0 = 0;
       long long kdone = 0;
+      RedGroup rg;
+      rg.c_off = x.P.c_off; rg.sts = x.P.c_tstride; rg.part_off = out.partial_elems; rg.ni = x.P.N; rg.M = x.P.M; rg.nparts = 0; rg.pad_ = 0;
       for (long long part = 0; part < parts; ++part) {
         const long long target = x.kt * (part + 1) / parts;
         gwsig_problem P = x.P;
+        if (deterministic) {            // private partial tile [M][N], plain stores; summed in part order afterwards
+          P.flags &= ~GWSIG_FLAG_ACCUM;
+          P.c_off = out.partial_elems;
+          P.cm = lvl1(x.P.N); P.cn = lvl1(1);
+          P.c_tstride = 0;
+        }
         P.seg_begin = (int)out.seg.size();
         long long kt = 0;
         while (s0 < x.segs.size() && (kdone < target || part == parts - 1)) {
@@ -512,7 +520,9 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
         P.seg_count = (int)out.seg.size() - P.seg_begin;
         if (P.seg_count == 0) continue;
         out.prob.push_back(P); cost.push_back(kt);
+        if (deterministic) { out.partial_elems += (long long)x.P.M * x.P.N; ++rg.nparts; }
       }
+      if (deterministic && rg.nparts > 0) out.red.push_back(rg);
     }
   }
 

@@ -14,7 +14,18 @@ namespace gwsig {
 
 typedef std::complex<double> cplx;
 
+// deterministic stage 3: the split-K parts of one Sigma block write private partial tiles [part][M][N] (contiguous),
+// summed into the accumulator in part order by reduce_parts_kernel
+struct RedGroup {
+  long long c_off;      // Sigma accumulator offset of the block (before t0 * sts)
+  long long sts;        // elements per tau in the accumulator
+  long long part_off;   // first partial tile in the scratch buffer
+  int ni, M, nparts, pad_;
+};
+
 struct StagePlan {
+  std::vector<RedGroup> red;      // only for stage 3 in deterministic mode
+  long long partial_elems = 0;
   std::vector<gwsig_problem> prob;
   std::vector<gwsig_seg> seg;
   std::vector<int> bucket;    // bucket[t >> 6] = problem holding tile (t & ~63)   (zgemm_grouped.cuh)
@@ -33,6 +44,7 @@ struct Plan {
 
   // ---- symmetry ---------------------------------------------------------------------------
   int nops = 0, mode = GWSIG_FULL_BZ;
+  bool deterministic = false;  // stage 3 without atomics: private partial tiles + an ordered reduction (option "deterministic")
   std::vector<int> rot;        // [nops][9]
   std::vector<double> trans;   // [nops][3]
   std::vector<double> D_ao, D_aux;

@@ -23,9 +23,10 @@ def _B():
     return binding
 
 
-def run_gpu(cfg, G, W, V, engine=0, pushes=None, scratch_mib=None, tau_chunk=None, hermitize=0):
+def run_gpu(cfg, G, W, V, engine=0, pushes=None, scratch_mib=None, tau_chunk=None, hermitize=0, deterministic=0):
     torch = _torch()
     lib = cfg.lib
+    lib.set_option("deterministic", deterministic)
     lib.set_option("engine", engine)
     lib.set_option("hermitize", hermitize)
     if scratch_mib:
@@ -225,6 +226,18 @@ def test_exchange_eq21c(name, mode):
     ref = oracle_exchange(inp, gam, ks)
     worst = max(rel_err(got[k][0], ref[a]) for a, k in enumerate(ks))
     assert worst <= TOL, worst
+
+
+def test_deterministic_accumulation_is_bit_reproducible():
+    """option "deterministic": the split-K parts of stage 3 go through private partial tiles and one ordered reduction instead
+    of FP64 atomics in scheduler order: two runs give bit-identical Sigma, and the result still matches the oracle."""
+    B, inp, cfg, G, W, V = _setup("cfg3", 2, mesh=(2, 2, 2), ntau=5)
+    a = run_gpu(cfg, G, W, V, deterministic=1, tau_chunk=2)
+    b = run_gpu(cfg, G, W, V, deterministic=1, tau_chunk=2)
+    assert np.array_equal(a.view(np.float64), b.view(np.float64))
+    _check(cfg, inp, a)
+    c = run_gpu(cfg, G, W, V, deterministic=0, tau_chunk=2)
+    assert np.abs(a - c).max() <= 1e-12 * np.abs(a).max()
 
 
 def test_output_point_subset_matches_full_run():
