@@ -47,10 +47,12 @@ typedef enum {
 } gwsig_mode;
 
 typedef enum {
-  GWSIG_ENGINE_DMMA = 0,      /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA), complex product by
-                                 the 3M / Karatsuba scheme: 3 real DMMA per complex 8x8x4 block (default)           */
+  GWSIG_ENGINE_DMMA = 0,      /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA), default: per stage the
+                                 faster of the two tensor kernels below (3M for stage 2, 4M for stages 1 and 3)         */
   GWSIG_ENGINE_REFERENCE = 1, /* one-thread-per-element DFMA kernels on the same plan (debug)                       */
-  GWSIG_ENGINE_DMMA_4M = 2    /* tensor-core kernel with the conventional 4-product complex multiply               */
+  GWSIG_ENGINE_DMMA_4M = 2,   /* every stage on the tensor-core kernel with the conventional 4-product complex multiply */
+  GWSIG_ENGINE_DMMA_3M = 3    /* every stage on the tensor-core kernel with the 3M / Karatsuba complex multiply:
+                                 3 real DMMA per complex 8x8x4 block                                                 */
 } gwsig_engine;
 
 /* kernel kinds for gwsig_kernel_times (steps a1..a6 of DESIGN.md) */
@@ -178,6 +180,9 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
  * default 8192), "tau_chunk" (0 = from the budget), "v_ring_mib" (size of one slot of the
  * V ring of sigma_eval_host, default 1024), "timing" (0/1: record a CUDA event pair around
  * every kernel launch on the launching stream, read back with gwsig_kernel_times),
+ * "bulk_copies" (0/1, default 0): 1 = the 3M kernel stages operands that are whole contiguous rows (stage 2: X, W;
+ * stage 3: V2) with cp.async.bulk (UBLKCP) instead of 16-byte cp.async -- measured slower on B200 (one bulk copy per 2 KB
+ * row issues at ~130 cycles), kept for comparison,
  * "deterministic" (0/1, default 0): 1 = the split-K parts of stage 3 write private partial tiles that are summed into
  * Sigma in a fixed order by a reduction kernel instead of FP64 atomics in scheduler order: results are then bit-identical
  * from run to run (same device, same options); costs one extra pass over the partial tiles                         */

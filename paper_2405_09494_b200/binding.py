@@ -17,7 +17,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 FULL_BZ, IBZ, IBZ_BLOCK = 0, 1, 2
-ENGINE_DMMA, ENGINE_REFERENCE, ENGINE_DMMA_4M = 0, 1, 2
+ENGINE_DMMA, ENGINE_REFERENCE, ENGINE_DMMA_4M, ENGINE_DMMA_3M = 0, 1, 2, 3
 NODIV = 0x7FFFFFFF
 FLAG_CONJ_A, FLAG_ACCUM, FLAG_A_KMAJOR, FLAG_CONJ_B = 1, 2, 4, 8
 

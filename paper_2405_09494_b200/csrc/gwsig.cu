@@ -62,6 +62,7 @@ struct gwsig_ctx {
   long long scratch_mib = 8192;
   long long v_ring_mib = 1024;
   int tau_chunk = 0;
+  int bulk_copies = 0;
   // evaluation state
   bool in_eval = false;
   bool exchange = false;        // evaluation opened by exchange_begin: no W, stage 2 skipped (Eq. 21c)
@@ -268,6 +269,17 @@ int toc(gwsig_ctx* ctx) {
   return GWSIG_OK;
 }
 
+// which kernel runs launch kind st (0 = Eq. 28 unfold, 1..3 = contraction stage) under engine option e:
+// GWSIG_ENGINE_DMMA (default) = the 3M kernel where it is the faster one on B200 (stage 2, 70 % of the flops: K = n_p up to
+// 116) and the 4-product kernel for the short-K stage 1, the narrow-N stage 3 and the unfold (measured)
+int stage_engine(int e, int st) {
+  if (e == GWSIG_ENGINE_DMMA) return st == 2 ? GWSIG_ENGINE_DMMA_3M : GWSIG_ENGINE_DMMA_4M;
+  return e;
+}
+void set_tile_heights(gwsig_ctx* ctx) {
+  for (int st = 0; st < 4; ++st) ctx->plan.tile_m[st] = stage_engine(ctx->engine, st) == GWSIG_ENGINE_DMMA_3M ? ZG_BM3 : ZG_BM;
+}
+
 int run_stage(gwsig_ctx* ctx, int kind, const DevStage& d, const double2* A, const double2* B, double2* C, int t0) {
   if (d.ntiles <= 0) return GWSIG_OK;
   if (ctx->counter_slot >= gwsig_ctx::kCounterSlots) {
@@ -282,10 +294,13 @@ int run_stage(gwsig_ctx* ctx, int kind, const DevStage& d, const double2* A, con
   zp.nprob = d.nprob;
   zp.total_tiles = d.ntiles;
   zp.t0 = t0;
+  zp.use_bulk = ctx->bulk_copies;
+  const int st = kind == GWSIG_KIND_STAGE1 ? 1 : kind == GWSIG_KIND_STAGE2 ? 2 : kind == GWSIG_KIND_STAGE3 ? 3 : 0;
+  zp.bm = ctx->plan.tile_m[st];
   zp.counter = (unsigned long long*)ctx->counters.p + ctx->counter_slot++;
   int rc = tic(ctx, kind);
   if (rc) return rc;
-  CU(zg_launch(ctx->engine, zp, ctx->num_sms, ctx->stream));
+  CU(zg_launch(stage_engine(ctx->engine, st), zp, ctx->num_sms, ctx->stream));
   if ((rc = toc(ctx))) return rc;
   ctx->launches++;
   return GWSIG_OK;
@@ -321,6 +336,14 @@ int run_block_unfold(gwsig_ctx* ctx, bool aux, int k_first, int k_count, const d
 
 }  // namespace
 
+static void invalidate(gwsig_ctx* ctx) {
+  ctx->tables_ready = false;
+  for (auto& kv : ctx->plan_cache)
+    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
+  ctx->plan_cache.clear();
+  ctx->in_eval = false;
+}
+
 // =============================================================================================
 extern "C" {
 
@@ -328,6 +351,7 @@ int gwsig_create(gwsig_ctx** out, int device) {
   if (!out) return GWSIG_ERR_ARG;
   *out = new gwsig_ctx();
   (*out)->device = device;
+  set_tile_heights(*out);
   return GWSIG_OK;
 }
 
@@ -356,13 +380,6 @@ int gwsig_destroy(gwsig_ctx* ctx) {
 
 const char* gwsig_last_error(const gwsig_ctx* ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
 
-static void invalidate(gwsig_ctx* ctx) {
-  ctx->tables_ready = false;
-  for (auto& kv : ctx->plan_cache)
-    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
-  ctx->plan_cache.clear();
-  ctx->in_eval = false;
-}
 
 int gwsig_set_lattice(gwsig_ctx* ctx, const double a[9], const int mesh[3], int nao, int naux, int ntau, double beta) {
   if (!ctx) return GWSIG_ERR_ARG;
@@ -459,12 +476,15 @@ int gwsig_set_option(gwsig_ctx* ctx, const char* key, int64_t value) {
   if (!ctx || !key) return GWSIG_ERR_ARG;
   std::string k(key);
   if (k == "engine") {
-    if (value != GWSIG_ENGINE_DMMA && value != GWSIG_ENGINE_REFERENCE && value != GWSIG_ENGINE_DMMA_4M) return fail(ctx, GWSIG_ERR_ARG, "set_option: bad engine");
+    if (value != GWSIG_ENGINE_DMMA && value != GWSIG_ENGINE_REFERENCE && value != GWSIG_ENGINE_DMMA_4M && value != GWSIG_ENGINE_DMMA_3M) return fail(ctx, GWSIG_ERR_ARG, "set_option: bad engine");
+    if (ctx->engine != (int)value) invalidate(ctx);       // the tile height is part of the plan
     ctx->engine = (int)value;
+    set_tile_heights(ctx);
   } else if (k == "hermitize") ctx->hermitize = value != 0;
   else if (k == "scratch_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: scratch_mib < 1"); ctx->scratch_mib = value; }
   else if (k == "v_ring_mib") { if (value < 1) return fail(ctx, GWSIG_ERR_ARG, "set_option: v_ring_mib < 1"); ctx->v_ring_mib = value; }
   else if (k == "timing") ctx->timing = value != 0;
+  else if (k == "bulk_copies") ctx->bulk_copies = value != 0;
   else if (k == "deterministic") { invalidate(ctx); ctx->plan.deterministic = value != 0; }
   else if (k == "tau_chunk") { if (value < 0) return fail(ctx, GWSIG_ERR_ARG, "set_option: tau_chunk < 0"); ctx->tau_chunk = (int)value; }
   else return fail(ctx, GWSIG_ERR_ARG, "set_option: unknown key " + k);

@@ -372,8 +372,8 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
           gwsig_seg S; std::memset(&S, 0, sizeof(S));
           gwsig_problem P; std::memset(&P, 0, sizeof(P));
           // X[P,i,b](tau) = sum_a conj(V2[P,a,i]) G[a,b](tau)          (Algorithm 4 line 5)
-          // lowered TRANSPOSED, X^T[(tau,b),(P,i)] = sum_a G^T[(tau,b),a] conj(V2)[a,(P,i)]: the 8 lanes of a fragment
-          // column then write 8 consecutive b of X (full 128-byte lines) and V2 is the narrow operand
+          // lowered TRANSPOSED, X^T[(tau,b),(P,i)] = sum_a G^T[(tau,b),a] conj(V2)[a,(P,i)]: tau folds into the long row
+          // index (each V2 tile is read once for all tau of the chunk) and V2 is the narrow operand
           S.a_off = goff + blk_off(ao_off[k2], L.al);
           S.am = lvl2(L.na, gts, 1);                      // m = (tau, b)
           S.ak = lvl1(L.na);                              // k = a
@@ -383,8 +383,11 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
           S.K = L.na;
           P.M = nt * L.na; P.N = L.np_ * L.ni;
           P.c_off = xoff[l] + L.poff + L.c0;
-          P.cm = lvl2(L.na, xs, 1);
-          P.cn = lvl2(L.ni, L.Np, L.na);
+          // X (and Y) segments are stored [P][b][i], i fastest -- the transpose of V2's [P][a][i] in the middle index only:
+          // every operand of every stage is then contiguous along its tile dimension (runs of n_alpha or n_iota elements,
+          // whole rows in stage 2), which is what the bulk-copy loader wants
+          P.cm = lvl2(L.na, xs, L.ni);
+          P.cn = lvl2(L.ni, L.Np, 1);
           P.a_tstride = gts;
           P.nbatch = 1;
           P.flags = GWSIG_FLAG_CONJ_B;
@@ -441,12 +444,12 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
         pair_layout(p, T, Np, poff, k1_, k2, q, i1_);
         const long long vrel = v_off[p] - v_off[p0];
         const long long xs = xsize(p);
-        if (xs * nt >= (1LL << 31)) return GWSIG_ERR_ARG;   // the k-major loader keeps 32-bit row offsets
+        if (xs * nt >= (1LL << 31)) return GWSIG_ERR_ARG;   // the per-element loader path keeps 32-bit row offsets
         for (const auto& L : T) {
           gwsig_seg S; std::memset(&S, 0, sizeof(S));
-          S.a_off = xoff[l] + L.poff + L.c0;               // Y, same layout as X
-          S.am = lvl2(L.ni, xs, L.na);                     // m = (tau, i)
-          S.ak = lvl2(L.na, L.Np, 1);                      // k = (P', b)
+          S.a_off = xoff[l] + L.poff + L.c0;               // Y, same layout as X: [P'][b][i]
+          S.am = lvl2(L.ni, xs, 1);                        // m = (tau, i)
+          S.ak = lvl2(L.na, L.Np, L.ni);                   // k = (P', b)
           S.b_off = vrel + L.poff + L.c0;
           S.bk = lvl2(L.na, L.Np, L.ni);
           S.bn = lvl1(1);
@@ -465,11 +468,11 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
         x.P.cm = lvl2(ni, sts, ni); x.P.cn = lvl1(1);
         x.P.c_tstride = sts;
         x.P.nbatch = 1;
-        x.P.flags = GWSIG_FLAG_ACCUM | GWSIG_FLAG_A_KMAJOR;
+        x.P.flags = GWSIG_FLAG_ACCUM;
         x.kt = 0;
         for (auto& S : segs[b]) x.kt += S.K;
         x.segs.swap(segs[b]);
-        tiles1 += (long long)zg_tiles_m(x.P.M) * zg_tiles_n(x.P.N);
+        tiles1 += (long long)zg_tiles_m(x.P.M, tile_m[3]) * zg_tiles_n(x.P.N);
         p3.push_back(std::move(x));
       }
     }
@@ -534,7 +537,7 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
   long long tb = 0;
   for (size_t i = 0; i < order.size(); ++i) {
     gwsig_problem P = out.prob[order[i]];
-    P.tiles_m = zg_tiles_m(P.M);
+    P.tiles_m = zg_tiles_m(P.M, tile_m[stage]);
     P.tiles_n = zg_tiles_n(P.N);
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
@@ -674,7 +677,7 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
   }
   long long tb = 0;
   for (auto& P : out.prob) {
-    P.tiles_m = zg_tiles_m(P.M);
+    P.tiles_m = zg_tiles_m(P.M, tile_m[0]);
     P.tiles_n = zg_tiles_n(P.N);
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;

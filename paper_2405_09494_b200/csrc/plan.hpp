@@ -44,6 +44,8 @@ struct Plan {
 
   // ---- symmetry ---------------------------------------------------------------------------
   int nops = 0, mode = GWSIG_FULL_BZ;
+  int tile_m[4] = {128, 128, 128, 128};   // tile height per launch kind: [0] Eq. 28 unfold, [1..3] contraction stage (the engine
+                                          // chosen for that stage fixes it: zgemm_grouped.cuh)
   bool deterministic = false;  // stage 3 without atomics: private partial tiles + an ordered reduction (option "deterministic")
   std::vector<int> rot;        // [nops][9]
   std::vector<double> trans;   // [nops][3]

@@ -2,10 +2,9 @@
 //
 // TWO tensor-core kernels share the loader, the tile scheduler and the descriptors:
 //   zgemm_grouped_dmma3m (engine 0, default): Karatsuba / "3M" complex product -- three REAL products
-//       P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi),  re = P1 - P2,  im = P3 - P1 - P2  (25 % fewer DMMA than 4M),
-//       one product per group of four MMA warps (12 MMA warps, 32 accumulator doubles each), accumulators handed to
-//       four EPILOGUE warps through shared memory so that the MMA warps never touch global memory or index arithmetic:
-//       loader warps -> MMA warps -> epilogue warps, decoupled by mbarriers (details above the kernel)
+//       P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi),  re = P1 - P2,  im = P3 - P1 - P2  (25 % fewer DMMA than 4M);
+//       16 MMA warps, one row group of the tile each, fed by ONE loader warp with bulk async copies (UBLKCP);
+//       details above the kernel
 //   zgemm_grouped_dmma   (engine 2): the conventional four-product kernel (engine v3 of round 1), described below.
 //
 // Serves the three contraction stages of the GW self-energy (Algorithm 4 lines 5, 7, 8 of
@@ -64,7 +63,7 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
   unsigned ok;
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared.b64 p, [%1], %2;\n\t"
+      "mbarrier.try_wait.parity.shared.b64 p, [%1], %2, 0x989680;\n\t"     // suspend-time hint: sleep in hardware, do not spin
       "selp.u32 %0, 1, 0, p;\n\t}\n"
       : "=r"(ok)
       : "r"(bar), "r"(parity)
@@ -434,160 +433,296 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
 }
 
 // ------------------------------------------------------------------------------------------
-// the 3M kernel: warps 0..11 MMA (three product groups of four), 12..15 loaders, 16..19 epilogue
+// the 3M kernel: warps 0..7 MMA, warps 8..9 loaders; two CTAs per SM
 //
 //   complex C += A B  as three real products (Karatsuba):  P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi),
-//   re C = P1 - P2,  im C = P3 - P1 - P2.  MMA warp (g, w) accumulates product g for row groups w, w+4, w+8, w+12
-//   of the 128-row tile and all (<= 4) column groups: 32 accumulator doubles.  Warp id mod 4 = w is the SM
-//   sub-partition, so every sub-partition hosts one warp of each product: three independent DMMA streams per FP64
-//   pipe.  conj(A) / conj(B): the sign of Ai / Bi enters the operand sums of P3 (XOR on the integer pipe) and the
-//   sign of P2 in the epilogue.  At the end of a tile the MMA warps drop their accumulators into a shared staging
-//   buffer [3][128][33] and go straight on with the next tile; the epilogue warps combine the three planes, do the
-//   two-level C addressing and store (or red.add) with full-line global accesses in the orientation C is
-//   contiguous in.  Register budget per CTA: 12 x 32 x 128 + 4 x 32 x 40 + 4 x 32 x 56 = 61440 = 640 x 96 at launch.
+//   re C = P1 - P2,  im C = P3 - P1 - P2:  3 real DMMA per complex 8x8x4 block instead of 4.
+//   MMA warp w owns row group w (8 rows) of the 64-row tile and all (<= 4) column groups, all three products: 24 accumulator
+//   doubles; it stores its own rows at the end of a tile (8 complex numbers per lane) and goes straight on.  conj(A) /
+//   conj(B) flip the sign of Ai / Bi on the integer pipe (XOR) before the operand sums.
+//   Two CTAs per SM (20 warps x 96 registers = the whole register file, no setmaxnreg): every SM sub-partition hosts two MMA
+//   warps of each CTA, and the two CTAs are at unrelated points of unrelated tiles, so one CTA's barrier round trips,
+//   fragment-load latency, tile switches and stores are covered by the other's DMMA stream (measured: sixteen MMA warps of
+//   ONE CTA run in lock step and leave the pipe idle at every step and slot boundary).
+//   Two loader warps per CTA feed a ring of kStages3 = 4 slots of BK3 = 16 k-rows (four k4 steps per barrier round trip,
+//   100 KB of shared memory per CTA).  The plan lays X and Y out so that every operand is contiguous along its tile dimension.
 // ------------------------------------------------------------------------------------------
-constexpr int kMmaWarps = 12;
-constexpr int kEpiWarps = 4;
-constexpr int kMmaRegs = 128, kLoaderRegs3 = 40, kEpiRegs = 56;
-constexpr int kThreads3 = (kMmaWarps + kProducerWarps + kEpiWarps) * 32;
-constexpr int kLaunchRegs3 = 96;                       // what __launch_bounds__(640, 1) gives every thread: 65536 / 640 -> 96
-// setmaxnreg only moves registers INSIDE the CTA's launch-time allocation: an inc beyond it waits forever
-static_assert(32 * (kMmaWarps * kMmaRegs + kProducerWarps * kLoaderRegs3 + kEpiWarps * kEpiRegs) <= kThreads3 * kLaunchRegs3,
-              "setmaxnreg budget exceeds the launch-time register allocation of the CTA");
-constexpr int STG_LD = ZG_BN + 1;                      // odd pitch (doubles): conflict-free in both epilogue orientations
-constexpr int kTrec3 = kStages + 3;                    // loaders <= kStages tiles ahead of the MMA warps, epilogue one behind
+constexpr int kMmaWarps = ZG_BM3 / 8;     // 8: one row group each
+constexpr int kLoaderWarps3 = 2;
+constexpr int LDA3 = ZG_BM3 + 2;          // = 2 (mod 8): conflict-free fragment loads
+static_assert(LDA3 % 8 == 2, "layout");
+constexpr int kThreads3 = (kMmaWarps + kLoaderWarps3) * 32;
+constexpr int BK3 = 16;
+constexpr int kStages3 = 4;
+constexpr int kTrec3 = kStages3 + 2;
+constexpr int kChunk3 = 4;             // consecutive tile ids a CTA takes per scheduler fetch
+constexpr unsigned kFullCount3 = 32 + 1;      // the 32 lanes of the slot's owner warp (cp.async-triggered arrive) + its lane 0's expect_tx
+static_assert(kStages3 % kLoaderWarps3 == 0, "loader warp lw owns ring stages lw, lw + kLoaderWarps3, ...");
 
-template <int MI, int NI>
-__device__ __forceinline__ void mma3_k4(double (&acc)[4][4][2], const double2* as, const double2* bs, int grp, unsigned sa,
-                                        unsigned sb) {
-  double2 af[MI], bf[NI];
-  double a[MI], b[NI];
-#pragma unroll
-  for (int i = 0; i < MI; ++i) af[i] = as[i * 32];
-#pragma unroll
-  for (int j = 0; j < NI; ++j) bf[j] = bs[j * 8];
-  if (grp == 0) {
-#pragma unroll
-    for (int i = 0; i < MI; ++i) a[i] = af[i].x;
-#pragma unroll
-    for (int j = 0; j < NI; ++j) b[j] = bf[j].x;
-  } else if (grp == 1) {
-#pragma unroll
-    for (int i = 0; i < MI; ++i) a[i] = af[i].y;
-#pragma unroll
-    for (int j = 0; j < NI; ++j) b[j] = bf[j].y;
-  } else {
-#pragma unroll
-    for (int i = 0; i < MI; ++i) a[i] = af[i].x + xor_hi(af[i].y, sa);
-#pragma unroll
-    for (int j = 0; j < NI; ++j) b[j] = bf[j].x + xor_hi(bf[j].y, sb);
-  }
-#pragma unroll
-  for (int i = 0; i < MI; ++i)
-#pragma unroll
-    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+__device__ __forceinline__ void bulk_g2s(unsigned smem_dst, const void* gmem_src, unsigned bytes, unsigned bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_dst),
+               "l"(gmem_src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared.b64 st, [%0], %1;\n\t}\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 
-template <int MI, int NI>
-__device__ __forceinline__ void mma3_slot(double (&acc)[4][4][2], const double2* as, const double2* bs, int nk4, int grp,
-                                          unsigned sa, unsigned sb) {
-#pragma unroll 1
-  for (int kk = 0; kk < nk4; ++kk) mma3_k4<MI, NI>(acc, as + kk * 4 * LDA, bs + kk * 4 * LDB, grp, sa, sb);
-}
-
-struct __align__(8) StageCtl {      // handshake MMA warps -> epilogue warps
-  int trec;                          // tile record of the staged tile
-  int ctl;                           // 4: no more tiles
+// step a two-level index by one: offset(i + 1) from offset(i) without a division
+struct KStep {
+  long long off, wrap;       // current offset; what to add when the fast index wraps (hi - div * lo)
+  long long lo;
+  int r, div;
 };
+__device__ __forceinline__ KStep kstep_init(const gwsig_idx2& d, int k) {
+  KStep s;
+  s.lo = d.lo; s.div = d.div;
+  if (d.div == GWSIG_NODIV) { s.r = 0; s.off = (long long)k * d.lo; s.wrap = 0; }
+  else { const int q = k / d.div; s.r = k - q * d.div; s.off = (long long)q * d.hi + (long long)s.r * d.lo; s.wrap = d.hi - (long long)d.div * d.lo; }
+  return s;
+}
+__device__ __forceinline__ void kstep_next(KStep& s) {        // branch-free: div = GWSIG_NODIV (INT_MAX) never wraps
+  const bool w = ++s.r == s.div;
+  s.off += s.lo + (w ? s.wrap : 0);
+  s.r = w ? 0 : s.r;
+}
+__device__ __forceinline__ void cp_async16_sz(unsigned smem_dst, const void* gmem_src, unsigned bytes) {   // bytes = 0: zero-fill, no read
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gmem_src), "r"(bytes) : "memory");
+}
 
-__global__ void __launch_bounds__(kThreads3, 1) zgemm_grouped_dmma3m(ZgParams p) {
+// Loader warp lw OWNS the ring slots whose global index is lw (mod kLoaderWarps3): every loader warp walks the same tile /
+// segment / slot sequence but only fills its own slots, so it has kLoaderWarps3 slot times for one slot's address
+// arithmetic.  Operands move as one 16-byte cp.async per element, lane <-> tile row / column (tile rows lane, lane + 32);
+// with ZgParams::use_bulk an operand whose tile dimension is ONE contiguous run (single-level index with unit stride: X / Y
+// and W rows in stage 2, V2 rows in stage 3) moves as one bulk copy per k-row instead, issued by lane 0 (UBLKCP).
+__device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2* Bs, unsigned full0, unsigned empty0, SlotHdr* hdr,
+                                        TileRec* trec, long long* next_tile, int lw, int lane) {
+  const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
+  const bool leader = lw == 0 && lane == 0;
+  int stage = 0, tslot = 0, tbuf = 0;
+  unsigned phase = 0;             // parity of the ring round of the next slot (all loader warps count alike)
+  int gslot = 0;                  // global slot index modulo kLoaderWarps3
+  long long pre = 0;
+  if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);
+  while (true) {
+    // tiles are taken kChunk3 consecutive ids at a time: neighbours belong to the same problem (n fastest), so their
+    // descriptor loads hit L1 and the chain of dependent L2 round trips is paid once per chunk, not once per tile
+    if (leader) next_tile[tbuf] = pre;
+    named_bar_sync(1, kLoaderWarps3 * 32);
+    const long long chunk0 = next_tile[tbuf] * kChunk3;
+    tbuf ^= 1;
+    if (chunk0 >= p.total_tiles) break;
+    if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);        // lands while this chunk is being staged
+    for (long long tile = chunk0; tile < chunk0 + kChunk3 && tile < p.total_tiles; ++tile) {
+      const TileInfo ti = decode_tile(p, tile);
+      const gwsig_problem& P = p.prob[ti.prob];
+      const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
+      const int m0 = ti.tm * ZG_BM3;
+      int n0, ncols;
+      zg_ntile(N, __ldg(&P.tiles_n), ti.tn, n0, ncols);
+      const int mrows = min(ZG_BM3, M - m0);
+      const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
+      const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
+      const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
+      bool first = true;
+      for (int s = 0; s < nseg; ++s) {
+        const gwsig_seg& S = p.seg[seg_begin + s];
+        const int K = __ldg(&S.K);
+        if (K == 0) continue;
+        const bool last_seg = s == nseg - 1;
+        const int nslots = (K + BK3 - 1) / BK3;
+        const int j0 = (lw - gslot + kLoaderWarps3) % kLoaderWarps3;       // this warp's first slot of the segment
+        if (j0 < nslots) {
+          const bool a_row = p.use_bulk && S.am.div == GWSIG_NODIV && S.am.lo == 1, b_row = p.use_bulk && S.bn.div == GWSIG_NODIV && S.bn.lo == 1;
+          const double2* abase = p.A + __ldg(&S.a_off) + a_boff + (a_row ? m0 : 0);
+          const double2* bbase = p.B + __ldg(&S.b_off) + b_boff + (b_row ? n0 : 0);
+          // per-lane source pointers of tile rows lane, lane + 32 and tile column lane; lanes outside the tile point at the
+          // operand base and copy zero bytes (cp.async zero-fills: no branch in the slot loop, nothing read)
+          const double2* pa[2];
+          unsigned sza[2], szb;
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const bool v = !a_row && lane + 32 * j < mrows;
+            pa[j] = abase + (v ? idx2(S.am, m0 + lane + 32 * j) : 0);
+            sza[j] = v ? 16u : 0u;
+          }
+          const bool vb = !b_row && lane < ncols;
+          const double2* pb = bbase + (vb ? idx2(S.bn, n0 + lane) : 0);
+          szb = vb ? 16u : 0u;
+          const gwsig_idx2 ak = S.ak, bk = S.bk;
+          for (int j = j0; j < nslots; j += kLoaderWarps3) {
+            const int k0 = j * BK3;
+            const int st = (stage + j) % kStages3;
+            const unsigned ph = phase ^ (unsigned)(((stage + j) / kStages3) & 1);     // ring round of this slot
+            const unsigned bar_full = full0 + 8 * st;
+            mbar_wait(empty0 + 8 * st, ph ^ 1);
+            const unsigned as = as0 + (unsigned)(st * BK3 * LDA3) * 16u, bs = bs0 + (unsigned)(st * BK3 * LDB) * 16u;
+            const int nkv = min(BK3, K - k0);                   // k-rows that hold data
+            const int nk4 = (nkv + 3) >> 2;
+            const bool firstslot = first && j == 0;
+            if (lane == 0) {                                    // slot header, then the releasing arrive that announces the bulk bytes
+              SlotHdr& h = hdr[st];
+              const bool last = last_seg && j == nslots - 1;
+              h.ctl = (firstslot ? 1 : 0) | (last ? 2 : 0);
+              h.nk4 = nk4;
+              if (firstslot) {
+                TileRec& t = trec[tslot];
+                t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
+                t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
+                t.cm = P.cm; t.cn = P.cn;
+                h.trec = tslot;
+              }
+              mbar_arrive_expect_tx(bar_full, (unsigned)(nkv * ((a_row ? mrows : 0) + (b_row ? ncols : 0)) * 16));
+            }
+            if (!a_row && !b_row && ak.div == GWSIG_NODIV && bk.div == GWSIG_NODIV) {
+              // stages 1 and 2: both k indices are single-level, three pointers advance by constant strides
+              const double2* qa0 = pa[0] + (long long)k0 * ak.lo;
+              const double2* qa1 = pa[1] + (long long)k0 * ak.lo;
+              const double2* qb = pb + (long long)k0 * bk.lo;
+              unsigned arow = as + (unsigned)lane * 16u, brow = bs + (unsigned)lane * 16u;
+              const long long sa_ = ak.lo, sb_ = bk.lo;
+#pragma unroll 4
+              for (int kk = 0; kk < 4 * nk4; ++kk) {
+                const bool kok = kk < nkv;
+                cp_async16_sz(arow, qa0, kok ? sza[0] : 0u);
+                cp_async16_sz(arow + 32u * 16u, qa1, kok ? sza[1] : 0u);
+                cp_async16_sz(brow, qb, kok ? szb : 0u);
+                arow += (unsigned)LDA3 * 16u; brow += (unsigned)LDB * 16u;
+                if (kok) { qa0 += sa_; qa1 += sa_; qb += sb_; }       // (never step past the last row: the pointers stay valid)
+              }
+              mbar_arrive_cp_async(bar_full);
+              continue;
+            }
+            KStep ka = kstep_init(ak, k0), kb = kstep_init(bk, k0);
+            if (!a_row && !b_row) {
+              // the common path: three cp.async per k-row and lane, no branches
+              unsigned arow = as + (unsigned)lane * 16u, brow = bs + (unsigned)lane * 16u;
+#pragma unroll 4
+              for (int kk = 0; kk < 4 * nk4; ++kk) {
+                const bool kok = kk < nkv;                      // rows of the last k4 step beyond K are zero-filled
+                cp_async16_sz(arow, pa[0] + ka.off, kok ? sza[0] : 0u);
+                cp_async16_sz(arow + 32u * 16u, pa[1] + ka.off, kok ? sza[1] : 0u);
+                cp_async16_sz(brow, pb + kb.off, kok ? szb : 0u);
+                arow += (unsigned)LDA3 * 16u; brow += (unsigned)LDB * 16u;
+                kstep_next(ka); kstep_next(kb);
+              }
+            } else {
+              for (int kk = 0; kk < 4 * nk4; ++kk) {
+                const bool kok = kk < nkv;
+                const unsigned arow = as + (unsigned)(kk * LDA3) * 16u, brow = bs + (unsigned)(kk * LDB) * 16u;
+                if (a_row) {
+                  if (kok) { if (lane == 0) bulk_g2s(arow, abase + ka.off, (unsigned)mrows * 16u, bar_full); }
+                  else for (int m = lane; m < mrows; m += 32) As[(st * BK3 + kk) * LDA3 + m] = make_double2(0.0, 0.0);
+                } else {
+                  cp_async16_sz(arow + (unsigned)lane * 16u, pa[0] + ka.off, kok ? sza[0] : 0u);
+                  cp_async16_sz(arow + (unsigned)(lane + 32) * 16u, pa[1] + ka.off, kok ? sza[1] : 0u);
+                }
+                if (b_row) {
+                  if (kok) { if (lane == 0) bulk_g2s(brow, bbase + kb.off, (unsigned)ncols * 16u, bar_full); }
+                  else if (lane < ncols) Bs[(st * BK3 + kk) * LDB + lane] = make_double2(0.0, 0.0);
+                } else {
+                  cp_async16_sz(brow + (unsigned)lane * 16u, pb + kb.off, kok ? szb : 0u);
+                }
+                kstep_next(ka); kstep_next(kb);
+              }
+            }
+            mbar_arrive_cp_async(bar_full);    // this lane's arrival, once its cp.async (if any) have landed; its zero stores precede it
+          }
+        }
+        if (first) { first = false; if (++tslot == kTrec3) tslot = 0; }
+        const int adv = stage + nslots;
+        phase ^= (unsigned)((adv / kStages3) & 1);
+        stage = adv % kStages3;
+        gslot = (gslot + nslots) % kLoaderWarps3;
+      }
+    }
+  }
+  // the slot after the last one carries the end mark: its owner tells the MMA warps there is no more work
+  if (lw == gslot) {
+    mbar_wait(empty0 + 8 * stage, phase ^ 1);
+    if (lane == 0) { hdr[stage].ctl = 4; mbar_arrive_expect_tx(full0 + 8 * stage, 0); }
+    mbar_arrive_cp_async(full0 + 8 * stage);
+  }
+  asm volatile("cp.async.wait_all;\n" ::: "memory");
+}
+
+// the k4 steps of one slot for one MMA warp: NI column groups, products P1, P2, P3 in acc[j][0..2].  The fragment registers
+// double as the P1 / P2 operands (sign flips in place), only the operand sums of P3 need registers of their own, so the warp
+// stays inside the 96 registers a 20-warp CTA gives every thread; P1 is issued before the operand sums so that the FP64 adds
+// queue behind the warp's own DMMAs, and the other three warps of the sub-partition cover the fragment-load latency.
+template <int NI>
+__device__ __forceinline__ void mma3_slot(double (&acc)[4][3][2], const double2* as, const double2* bs, int nk4, unsigned sa, unsigned sb) {
+#pragma unroll 1
+  for (int kk = 0; kk < nk4; ++kk) {
+    double2 af = as[kk * 4 * LDA3], bf[NI];
+#pragma unroll
+    for (int j = 0; j < NI; ++j) bf[j] = bs[kk * 4 * LDB + j * 8];
+    af.y = xor_hi(af.y, sa);
+#pragma unroll
+    for (int j = 0; j < NI; ++j) bf[j].y = xor_hi(bf[j].y, sb);
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[j][0][0], acc[j][0][1], af.x, bf[j].x);
+    const double asum = af.x + af.y;
+    double bsum[NI];
+#pragma unroll
+    for (int j = 0; j < NI; ++j) bsum[j] = bf[j].x + bf[j].y;
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[j][1][0], acc[j][1][1], af.y, bf[j].y);
+#pragma unroll
+    for (int j = 0; j < NI; ++j) dmma884(acc[j][2][0], acc[j][2][1], asum, bsum[j]);
+  }
+}
+
+// accumulators of one row group -> C: re = P1 - P2, im = P3 - P1 - P2; lane (fr, fk) holds row fr, columns 8 j + 2 fk + c
+__device__ __forceinline__ void store_rows3(const double (&acc)[4][3][2], const TileRec& t, double2* C, int rg, int lane) {
+  const int fr = lane >> 2, fk = lane & 3;
+  double2* cbase = C + t.c_off;
+  const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
+  const long long my_col = lane < t.ncols ? idx2(t.cn, t.n0 + lane) : -1;
+  const int row = rg * 8 + fr;
+  const long long roff = row < t.mrows ? idx2(t.cm, t.m0 + row) : -1;
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const long long coff = __shfl_sync(0xffffffffu, my_col, j * 8 + fk * 2 + c);
+      if (roff >= 0 && coff >= 0) {
+        const double re = acc[j][0][c] - acc[j][1][c], im = acc[j][2][c] - acc[j][0][c] - acc[j][1][c];
+        double2* dst = cbase + roff + coff;
+        if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
+        else *dst = make_double2(re, im);
+      }
+    }
+}
+
+__global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p) {
   extern __shared__ double2 zg_smem[];
-  double2* As = zg_smem;                             // [kStages][BK][LDA]
-  double2* Bs = zg_smem + kStages * BK * LDA;        // [kStages][BK][LDB]
-  double* Stg = reinterpret_cast<double*>(zg_smem + kStages * BK * (LDA + LDB));   // [3][ZG_BM][STG_LD]
-  __shared__ __align__(8) unsigned long long bars[2 * kStages + 2];
-  __shared__ SlotHdr hdr[kStages];
+  double2* As = zg_smem;                              // [kStages3][BK3][LDA3]
+  double2* Bs = zg_smem + kStages3 * BK3 * LDA3;      // [kStages3][BK3][LDB]
+  __shared__ __align__(8) unsigned long long bars[2 * kStages3];
+  __shared__ SlotHdr hdr[kStages3];
   __shared__ TileRec trec[kTrec3];
   __shared__ long long next_tile[2];
-  __shared__ StageCtl sctl;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
-  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[kStages]);
-  const unsigned stg_full = (unsigned)__cvta_generic_to_shared(&bars[2 * kStages]);
-  const unsigned stg_empty = (unsigned)__cvta_generic_to_shared(&bars[2 * kStages + 1]);
+  const unsigned empty0 = (unsigned)__cvta_generic_to_shared(&bars[kStages3]);
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, kProducerWarps * 32 + 1); mbar_init(empty0 + 8 * s, kMmaWarps); }
-    mbar_init(stg_full, kMmaWarps);
-    mbar_init(stg_empty, kEpiWarps);
+    for (int s = 0; s < kStages3; ++s) { mbar_init(full0 + 8 * s, kFullCount3); mbar_init(empty0 + 8 * s, kMmaWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
 
-  if (warp >= kMmaWarps + kProducerWarps) {
-    // ================================= EPILOGUE WARPS ===========================================
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kEpiRegs));
-    const int ew = warp - kMmaWarps - kProducerWarps;
-    unsigned tpar = 0;
-    while (true) {
-      mbar_wait(stg_full, tpar);
-      if (sctl.ctl & 4) break;
-      const TileRec& t = trec[sctl.trec];
-      const int mrows = t.mrows, ncols = t.ncols;
-      const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
-      const bool flip = ((t.flags & GWSIG_FLAG_CONJ_A) != 0) != ((t.flags & GWSIG_FLAG_CONJ_B) != 0);   // sign of Ai Bi
-      double2* cbase = p.C + t.c_off;
-      const int row = 32 * ew + lane;
-      const long long my_roff = row < mrows ? idx2(t.cm, t.m0 + row) : -1;
-      const long long my_coff = lane < ncols ? idx2(t.cn, t.n0 + lane) : -1;
-      const double* s1 = Stg, *s2 = Stg + ZG_BM * STG_LD, *s3 = Stg + 2 * ZG_BM * STG_LD;
-      if (t.cm.lo == 1) {
-        // C contiguous along m (X, Y): lane <-> row, walk the columns; 32 lanes write 32 consecutive rows
-        const double* q1 = s1 + row * STG_LD, *q2 = s2 + row * STG_LD, *q3 = s3 + row * STG_LD;
-        for (int c = 0; c < ncols; ++c) {
-          const long long coff = __shfl_sync(0xffffffffu, my_coff, c);
-          if (my_roff >= 0) {
-            const double p1 = q1[c], p2 = flip ? -q2[c] : q2[c], p3 = q3[c];
-            const double re = p1 - p2, im = p3 - p1 - p2;
-            double2* dst = cbase + my_roff + coff;
-            if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
-            else *dst = make_double2(re, im);
-          }
-        }
-      } else {
-        // C contiguous along n (Sigma blocks): lane <-> column, walk this warp's 32 rows
-        const int rend = min(32, mrows - 32 * ew);
-        for (int rr = 0; rr < rend; ++rr) {
-          const long long roff = __shfl_sync(0xffffffffu, my_roff, rr);
-          if (my_coff >= 0) {
-            const int r = 32 * ew + rr;
-            const double p1 = s1[r * STG_LD + lane], p2r = s2[r * STG_LD + lane], p3 = s3[r * STG_LD + lane];
-            const double p2 = flip ? -p2r : p2r;
-            const double re = p1 - p2, im = p3 - p1 - p2;
-            double2* dst = cbase + roff + my_coff;
-            if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
-            else *dst = make_double2(re, im);
-          }
-        }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(stg_empty);
-      tpar ^= 1;
-    }
-  } else if (warp >= kMmaWarps) {
-    // ================================= LOADER WARPS =============================================
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(kLoaderRegs3));
-    RingCtl rc;
-    rc.full0 = full0; rc.empty0 = empty0; rc.hdr = hdr; rc.trec = trec; rc.ntrec = kTrec3; rc.next_tile = next_tile;
-    producer_loop(p, As, Bs, rc, warp - kMmaWarps, lane);
+  if (warp >= kMmaWarps) {
+    loader3(p, As, Bs, full0, empty0, hdr, trec, next_tile, warp - kMmaWarps, lane);
   } else {
     // ================================= MMA WARPS ================================================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(kMmaRegs));
-    const int grp = warp >> 2, wq = warp & 3;
     const int fr = lane >> 2, fk = lane & 3;
-    double acc[4][4][2];
-    int stage = 0, tslot = 0, variant = -1, mi = 0, ng = 0;
-    unsigned phase = 0, tpar = 0, sa = 0, sb = 0;
+    double acc[4][3][2];
+    int stage = 0, tslot = 0, ng = 0;
+    bool active = false;
+    unsigned phase = 0, sa = 0, sb = 0;
     while (true) {
       mbar_wait(full0 + 8 * stage, phase);
       const int ctl = hdr[stage].ctl;
@@ -595,52 +730,29 @@ __global__ void __launch_bounds__(kThreads3, 1) zgemm_grouped_dmma3m(ZgParams p)
       if (ctl & 1) {
         tslot = hdr[stage].trec;
         const TileRec& t = trec[tslot];
-        const int mg = (t.mrows + 7) >> 3;
+        active = warp * 8 < t.mrows;
         ng = (t.ncols + 7) >> 3;
-        mi = mg > wq ? (mg - wq + 3) >> 2 : 0;
-        variant = mi > 0 ? (mi - 1) * 4 + (ng - 1) : -1;
         sa = (t.flags & GWSIG_FLAG_CONJ_A) ? 0x80000000u : 0u;
         sb = (t.flags & GWSIG_FLAG_CONJ_B) ? 0x80000000u : 0u;
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j)
 #pragma unroll
-          for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+          for (int q = 0; q < 3; ++q) { acc[j][q][0] = 0.0; acc[j][q][1] = 0.0; }
       }
-      if (variant >= 0) {
-        const double2* as = As + stage * BK * LDA + fk * LDA + wq * 8 + fr;
-        const double2* bs = Bs + stage * BK * LDB + fk * LDB + fr;
+      if (active) {
+        const double2* as = As + stage * BK3 * LDA3 + fk * LDA3 + warp * 8 + fr;
+        const double2* bs = Bs + stage * BK3 * LDB + fk * LDB + fr;
         const int nk4 = hdr[stage].nk4;
-#define ZG_F(MI_, NI_) mma3_slot<MI_, NI_>(acc, as, bs, nk4, grp, sa, sb);
-        switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
-#undef ZG_F
+        if (ng == 4) mma3_slot<4>(acc, as, bs, nk4, sa, sb);
+        else if (ng == 3) mma3_slot<3>(acc, as, bs, nk4, sa, sb);
+        else if (ng == 2) mma3_slot<2>(acc, as, bs, nk4, sa, sb);
+        else mma3_slot<1>(acc, as, bs, nk4, sa, sb);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-      if (++stage == kStages) { stage = 0; phase ^= 1; }
-
-      if (ctl & 2) {
-        // ---- hand the accumulators of this product to the epilogue warps -----------------------
-        mbar_wait(stg_empty, tpar ^ 1);                 // staging buffer free (passes at once for the first tile)
-        double* sg = Stg + grp * (ZG_BM * STG_LD) + (wq * 8 + fr) * STG_LD + 2 * fk;
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            if (i < mi && j < ng) {
-              sg[i * 32 * STG_LD + j * 8] = acc[i][j][0];
-              sg[i * 32 * STG_LD + j * 8 + 1] = acc[i][j][1];
-            }
-        if (warp == 0 && lane == 0) { sctl.trec = tslot; sctl.ctl = 0; }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(stg_full);
-        tpar ^= 1;
-      }
+      if (++stage == kStages3) { stage = 0; phase ^= 1; }
+      if ((ctl & 2) && active) store_rows3(acc, trec[tslot], p.C, warp, lane);
     }
-    // no more tiles: release the epilogue warps
-    mbar_wait(stg_empty, tpar ^ 1);
-    if (warp == 0 && lane == 0) sctl.ctl = 4;
-    __syncwarp();
-    if (lane == 0) mbar_arrive(stg_full);
   }
 }
 
@@ -657,7 +769,7 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
     double2* cbase = p.C + P.c_off + (long long)ti.batch * P.c_bstride + (long long)p.t0 * P.c_tstride;
     int n0, ncols;
     zg_ntile(P.N, P.tiles_n, ti.tn, n0, ncols);
-    const int m0 = ti.tm * ZG_BM, mrows = min(ZG_BM, P.M - m0);
+    const int m0 = ti.tm * p.bm, mrows = min(p.bm, P.M - m0);
     for (int e = threadIdx.x; e < mrows * ncols; e += blockDim.x) {
       int m = m0 + e / ncols, n = n0 + e % ncols;
       double sr = 0.0, si = 0.0;
@@ -683,7 +795,7 @@ __global__ void __launch_bounds__(256) zgemm_grouped_reference(ZgParams p) {
 }  // namespace
 
 namespace {
-struct LaunchCfg { bool ok3 = false, ok4 = false; int occ4 = 1; };
+struct LaunchCfg { bool ok3 = false, ok4 = false; int occ3 = 1, occ4 = 1; };
 LaunchCfg g_cfg[64];                 // per device: the shared-memory opt-in is a per-device function attribute
 std::mutex g_cfg_mu;
 }  // namespace
@@ -701,16 +813,23 @@ cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t s
   if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
   std::lock_guard<std::mutex> lk(g_cfg_mu);
   LaunchCfg& cfg = g_cfg[dev];
-  if (engine == 0) {
-    // 3M kernel: 12 MMA + 4 loader + 4 epilogue warps, one persistent CTA per SM
-    constexpr int smem = kStages * BK * (LDA + LDB) * (int)sizeof(double2) + 3 * ZG_BM * STG_LD * (int)sizeof(double);
+  if (engine == 3) {
+    // 3M kernel: 8 MMA + 2 loader warps, two persistent CTAs per SM (96 registers per thread), 64-row tiles
+    constexpr int smem = kStages3 * BK3 * (LDA3 + LDB) * (int)sizeof(double2);
+    if (p.bm != ZG_BM3) return cudaErrorInvalidValue;
     if (!cfg.ok3) {
       e = cudaFuncSetAttribute(zgemm_grouped_dmma3m, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
       if (e != cudaSuccess) return e;
+      e = cudaFuncSetAttribute(zgemm_grouped_dmma3m, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+      if (e != cudaSuccess) return e;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cfg.occ3, zgemm_grouped_dmma3m, kThreads3, smem);
+      if (e != cudaSuccess) return e;
+      if (cfg.occ3 < 1) cfg.occ3 = 1;
       cfg.ok3 = true;
     }
-    long long grid = num_sms;
-    if (grid > p.total_tiles) grid = p.total_tiles;
+    long long nchunks = (p.total_tiles + kChunk3 - 1) / kChunk3;
+    long long grid = (long long)num_sms * cfg.occ3;
+    if (grid > nchunks) grid = nchunks;
     if (grid < 1) return cudaSuccess;
     zgemm_grouped_dmma3m<<<(unsigned)grid, kThreads3, smem, stream>>>(p);
     return cudaGetLastError();
@@ -718,6 +837,7 @@ cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t s
   // 4M kernel: 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 200 / 56
   constexpr int smem = kStages * BK * (LDA + LDB) * (int)sizeof(double2);
   constexpr int threads = (kConsumerWarps + kProducerWarps) * 32;
+  if (p.bm != ZG_BM) return cudaErrorInvalidValue;
   if (!cfg.ok4) {
     e = cudaFuncSetAttribute(zgemm_grouped_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;

@@ -13,16 +13,17 @@
 #endif
 
 // ---- tiling rule -----------------------------------------------------------------------------------------
-// A problem C[M x N] is cut into tiles of ZG_BM = 128 rows and of at most ZG_NG_MAX = 4 column groups of 8:
+// A problem C[M x N] is cut into tiles of bm rows (ZG_BM = 128 or ZG_BM3 = 64, by engine) and of at most ZG_NG_MAX = 4 column groups of 8:
 // the G = ceil(N / 8) column groups are dealt evenly to tiles_n = ceil(G / 4) tiles (tile j owns groups
 // [j G / tiles_n, (j + 1) G / tiles_n)), so a ragged N costs no tensor-pipe time beyond its last group of 8.
 // Tiles of a problem are numbered batch-major, then m, then n (n fastest).
-constexpr int ZG_BM = 128;
+constexpr int ZG_BM = 128;                // tile height of the 4-product kernel (and the default of the plan)
+constexpr int ZG_BM3 = 64;                // tile height of the 3M kernel (two CTAs per SM, eight MMA warps each)
 constexpr int ZG_NG_MAX = 4;
 constexpr int ZG_BN = 8 * ZG_NG_MAX;
 constexpr int ZG_BUCKET_SHIFT = 6;        // tile -> problem lookup: one table entry per 64 tiles
 
-ZG_HD int zg_tiles_m(int M) { return (M + ZG_BM - 1) / ZG_BM; }
+ZG_HD int zg_tiles_m(int M, int bm) { return (M + bm - 1) / bm; }
 ZG_HD int zg_tiles_n(int N) { return ((N + 7) / 8 + ZG_NG_MAX - 1) / ZG_NG_MAX; }
 ZG_HD void zg_ntile(int N, int tiles_n, int tn, int& n0, int& ncols) {
   const int G = (N + 7) / 8;
@@ -42,6 +43,8 @@ struct ZgParams {
   int nprob;
   long long total_tiles;
   int t0;                      // first tau of the chunk (multiplies *_tstride)
+  int bm;                      // tile height the plan was built for (ZG_BM or ZG_BM3)
+  int use_bulk;                // 3M kernel: move whole-row operands with cp.async.bulk (UBLKCP) instead of 16-byte cp.async
   unsigned long long* counter; // device, zeroed before launch (dynamic tile scheduler)
 };
 

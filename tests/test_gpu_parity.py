@@ -81,7 +81,7 @@ def _setup(name, mode, **over):
     return B, inp, cfg, G, W, V
 
 
-@pytest.mark.parametrize("engine", [1, 0, 2])
+@pytest.mark.parametrize("engine", [1, 0, 2, 3])
 def test_cfg1_full_bz(engine):
     """BASELINE.json config 1, whole output."""
     B, inp, cfg, G, W, V = _setup("cfg1", 0)
@@ -99,7 +99,7 @@ def test_cfg1_ragged_and_chunked():
 @pytest.mark.parametrize("mode", [1, 2])
 def test_toys_ibz_and_block(name, mode):
     B, inp, cfg, G, W, V = _setup(name, mode)
-    for engine in (1, 0, 2):
+    for engine in (1, 0, 2, 3):
         _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
     _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=1))
 
@@ -168,8 +168,9 @@ def test_engine_variants_are_all_exercised():
     hit = set()
     for nao, naux, ntau in _VARIANT_CASES:
         B, inp, cfg, G, W, V = _setup("cfg1", 0, mesh=(2, 1, 1), nao=nao, naux=naux, ntau=ntau, beta=3.0, nocc=max(1, nao // 2), seed=nao)
+        cfg.lib.set_option("engine", 2)              # the 4-product kernel's 128-row tiling (its main loop has the 16 variants)
         hit |= _variants_hit(cfg)
-        for engine in (0, 2):
+        for engine in (0, 2, 3):
             _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
     assert hit == {(mi, ni) for mi in range(1, 5) for ni in range(1, 5)}, sorted(hit)
 
@@ -179,7 +180,7 @@ def test_cfg3_shaped_small_mesh_full_oracle():
     multiple of 4, stage-3 segment lists cut along P') on a 2x2x2 mesh with 5 tau points, where the oracle can check EVERY
     (k, tau) of the zone: block mode with both tensor kernels, IBZ mode, several pushes and tau chunks."""
     B, inp, cfg, G, W, V = _setup("cfg3", 2, mesh=(2, 2, 2), ntau=5)
-    for engine in (0, 2):
+    for engine in (0, 2, 3):
         _check(cfg, inp, run_gpu(cfg, G, W, V, engine=engine))
     _check(cfg, inp, run_gpu(cfg, G, W, V, pushes=cfg.nk1 * 3, tau_chunk=2))
     B, inp, cfg, G, W, V = _setup("cfg3", 1, mesh=(2, 2, 2), ntau=5)
