@@ -230,6 +230,12 @@ int get_dev_plan(gwsig_ctx* ctx, long long p0, long long np, int nt, int q_first
   auto key = std::make_tuple(p0, np, nt, q_first);
   auto it = ctx->plan_cache.find(key);
   if (it != ctx->plan_cache.end()) { *out = it->second.get(); return GWSIG_OK; }
+  if (ctx->plan_cache.size() >= 256) {          // callers that push ever-changing ranges must not grow the cache without bound
+    CU(cudaStreamSynchronize(ctx->stream));      // (a cached plan may still be read by kernels in flight)
+    for (auto& kv : ctx->plan_cache)
+      for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
+    ctx->plan_cache.clear();
+  }
   std::unique_ptr<DevPlan> dp(new DevPlan());
   for (int s = 0; s < 3; ++s) {
     StagePlan sp;
@@ -615,7 +621,11 @@ int gwsig_sigma_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* d
   const double2* Gsrc = (P.mode == GWSIG_IBZ || blk_unfold) ? (const double2*)ctx->gbz.p : ctx->dG;
 
   // sub-batches of pairs (whole q's where possible) and tau chunks sized to the scratch budget
-  const double budget = (double)ctx->scratch_mib * 1048576.0 / (2.0 * sizeof(double2));   // elements of X (= of Y)
+  // X + Y scratch: the option, but never more than 40 % of what the device has free (+ what the scratch already holds)
+  size_t free_b = 0, total_b = 0;
+  CU(cudaMemGetInfo(&free_b, &total_b));
+  const double avail = 0.4 * ((double)free_b + (double)ctx->xbuf.bytes + (double)ctx->ybuf.bytes);
+  const double budget = std::min((double)ctx->scratch_mib * 1048576.0, std::max(avail, 64.0 * 1048576.0)) / (2.0 * sizeof(double2));   // elements of X (= of Y)
   long long s0 = p0;
   while (s0 < p0 + np) {
     // grow the sub-batch by whole q's while X for all tau still fits

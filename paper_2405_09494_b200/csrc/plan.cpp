@@ -529,6 +529,25 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
     }
   }
 
+  // range checks the kernels rely on: element offsets of A inside a tile fit 32 bits (the 4-product kernel keeps them in int),
+  // a problem has fewer than 2^31 tiles, every problem has work (a C = tile without any K would never be written)
+  auto span = [](const gwsig_idx2& d, long long n) -> long long {
+    if (n <= 0) return 0;
+    if (d.div == GWSIG_NODIV) return (n - 1) * d.lo;
+    return ((n - 1) / d.div) * d.hi + std::min<long long>(d.div - 1, n - 1) * d.lo;
+  };
+  for (const auto& P : out.prob) {
+    long long ktot = 0;
+    for (int s = P.seg_begin; s < P.seg_begin + P.seg_count; ++s) {
+      const gwsig_seg& S = out.seg[s];
+      ktot += S.K;
+      if (span(S.am, P.M) >= (1LL << 31) || span(S.bn, P.N) >= (1LL << 31)) { return GWSIG_ERR_ARG; }
+    }
+    if (ktot <= 0) return GWSIG_ERR_ARG;
+    const long long nt_ = (long long)P.nbatch * zg_tiles_m(P.M, tile_m[stage]) * zg_tiles_n(P.N);
+    if (nt_ >= (1LL << 31)) return GWSIG_ERR_ARG;
+  }
+
   // heaviest problems first (dynamic scheduler takes tiles in order), then the tile prefix and the bucket table
   std::vector<int> order(out.prob.size());
   std::iota(order.begin(), order.end(), 0);

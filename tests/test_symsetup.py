@@ -153,3 +153,35 @@ def test_device_blocker_matches_block_V2():
         got = dst[off[r]:off[r + 1]].numpy()
         assert got.shape == packed_ref.shape
         assert np.abs(got - packed_ref).max() <= 1e-13 * vmax
+
+
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite", "toy_rocksalt"])
+def test_allowed_triples_do_not_depend_on_the_threshold(name):
+    """the allowed (p, alpha, iota) blocks are found by block max-abs > thresh * max|V| (S6): symmetry-forbidden blocks are
+    zero to rounding (~1e-16), allowed ones are O(1e-2..1) of max|V| for the synthetic V, so any threshold in between gives
+    the same list -- a small allowed block is not silently dropped, a rounding-level forbidden one not kept."""
+    from paper_2405_09494_b200 import binding as B
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    inp = make_inputs(name)
+    cfg = configure_from_crystal(B.Gwsig(device=-1), inp.cr, B.IBZ_BLOCK)
+    smallest_kept, largest_dropped = np.inf, 0.0
+    for p in range(0, cfg.npairs, max(1, cfg.npairs // 40)):
+        k1, k2, q, _, _ = cfg.lib.pair_info(p, with_layout=False)
+        V2 = inp.V2_rows(k1, [k2])[0]
+        vmax = np.abs(V2).max()
+        lists = [cfg.setup.block_V2(V2, k1, k2, cfg.ao, cfg.aux, thresh=t, vmax=vmax)[0] for t in (1e-5, 1e-9, 1e-12)]
+        assert np.array_equal(lists[0], lists[1]) and np.array_equal(lists[1], lists[2])
+        # the gap between kept and dropped blocks
+        T = np.einsum("QP,Qbj->Pbj", cfg.aux.U[q].conj(), V2)
+        T = np.einsum("ba,Pbj->Paj", cfg.ao.U[k2].conj(), T) @ cfg.ao.U[k1]
+        op, o2, o1 = cfg.aux.off[q], cfg.ao.off[k2], cfg.ao.off[k1]
+        kept = {tuple(t) for t in lists[1]}
+        for a in range(len(op) - 1):
+            for b in range(len(o2) - 1):
+                for c in range(len(o1) - 1):
+                    m = np.abs(T[op[a]:op[a + 1], o2[b]:o2[b + 1], o1[c]:o1[c + 1]]).max() / vmax
+                    if (a, b, c) in kept:
+                        smallest_kept = min(smallest_kept, m)
+                    else:
+                        largest_dropped = max(largest_dropped, m)
+    assert largest_dropped < 1e-13 and smallest_kept > 1e-4, (largest_dropped, smallest_kept)
