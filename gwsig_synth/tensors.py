@@ -145,10 +145,8 @@ def _group_average(cr: Crystal, keys: np.ndarray, M: np.ndarray, reps, starts, n
     multiplied by the real representation matrix ``reps[j][g]`` (perm (x) Wigner D).
     The representation matrices only connect atom x to perm x, so each atom block
     is transformed on its own with the matching sub-matrices (same result as
-    transforming the whole tensor, a fraction of the work); operations run on a
-    small thread pool, the accumulation into the output is serialised."""
+    transforming the whole tensor, a fraction of the work)."""
     import threading
-    from concurrent.futures import ThreadPoolExecutor
     sg = cr.sg
     nat = cr.natom
     nR = nleg - 1
@@ -187,9 +185,10 @@ def _group_average(cr: Crystal, keys: np.ndarray, M: np.ndarray, reps, starts, n
                 out_keys[idx] = nk_
                 out[(idx,) + sout] += B
 
-    nthreads = max(1, min(4, (os.cpu_count() or 1) // 2))
-    with ThreadPoolExecutor(nthreads) as pool:
-        list(pool.map(one_op, range(sg.nops)))
+    # serial over the operations: concurrent calls into the multi-threaded BLAS from several Python threads corrupted the
+    # result for the larger bases (config 5: V lost its transposition symmetry); the BLAS calls are threaded by themselves
+    for g in range(sg.nops):
+        one_op(g)
     out /= sg.nops
     keep = np.abs(out).reshape(len(uniq), -1).max(axis=1) > 0
     if keep.all():

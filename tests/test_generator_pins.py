@@ -161,3 +161,22 @@ def test_cfg1_recipe():
     assert np.abs(inp.V_pair(5, 2) - V.conj().transpose(0, 2, 1)).max() == 0
     assert np.abs(inp.V_pair(3, 3) - inp.V_pair(3, 3).conj().transpose(0, 2, 1)).max() < 1e-15
     assert abs(V.real.std() * np.sqrt(32) - 1) < 0.05 and abs(V.imag.std() * np.sqrt(32) - 1) < 0.05
+
+
+def test_three_centre_table_symmetric_at_a_large_basis():
+    """the group-averaged real-space V keeps V_{Q,j,i}(R2,R1) = V_{Q,i,j}(R1,R2) (G8) and Eq. 24a also at a basis large enough
+    for the BLAS to run multi-threaded (nao 58: config 5's orbital shells) -- a threaded version of the averaging once lost
+    both there while every small crystal passed."""
+    inp = make_inputs("cfg5", mesh=(2, 2, 2), ntau=2, aux=["s1 p1 d1"] * 2)
+    na, no = inp.naux, inp.nao
+    i1 = {tuple(R): i for i, R in enumerate(inp.vR1)}
+    i2 = {tuple(R): i for i, R in enumerate(inp.vR2)}
+    worst = 0.0
+    for R1 in inp.vR1[::5]:
+        for R2 in inp.vR2[::7]:
+            A = inp.Vd[i1[tuple(R1)], i2[tuple(R2)]].reshape(na, no, no)
+            Bm = inp.Vd[i1[tuple(R2)], i2[tuple(R1)]].reshape(na, no, no)
+            worst = max(worst, np.abs(A - Bm.transpose(0, 2, 1)).max())
+    assert worst <= 1e-14 * np.abs(inp.Vd).max()
+    a, b = inp.V2_rows(3, [5])[0], inp.V1_rows(3, [5])[0]
+    assert np.abs(a - b.conj().transpose(0, 2, 1)).max() <= 1e-13 * np.abs(a).max()
