@@ -125,6 +125,47 @@ def _setup_full_from_crystal(name):
     return B, inp, cfg, G, W, V
 
 
+def _pack_V_device(cfg, inp, batch=64):
+    """block-mode packing of V for the large configs with the batched GPU pre-step (presetup_device.DeviceBlocker: Eq. 27
+    transform, allowed-block detection, packing; checked against the per-pair numpy pre-step symsetup.block_V2 in
+    tests/test_symsetup.py) -- the per-pair Python loop of cfg.pack_V costs minutes at config 5.  Dense V rows still come from
+    the numpy generator."""
+    torch = _torch()
+    from paper_2405_09494_b200.presetup_device import DeviceBlocker
+    lib, nk1 = cfg.lib, cfg.nk1
+    blk = DeviceBlocker(cfg, torch, torch.device("cuda"))
+    k2_of = lambda p: lib.pair_info(p, with_layout=False)[1]
+    dense = {}
+    for i1, k1 in enumerate(cfg.out_list):
+        k2s = [k2_of(q * nk1 + i1) for q in range(cfg.nk)]
+        dense[i1] = inp.V2_rows(int(k1), k2s)                    # [nk, naux, nao, nao], row q
+    vmax = float(np.abs(dense[0]).max())
+    pairs = list(range(cfg.npairs))
+    info = [(p // nk1, k2_of(p), int(cfg.out_list[p % nk1])) for p in pairs]
+    trip, Ts = [], []
+    for b0 in range(0, cfg.npairs, batch):
+        pb = pairs[b0:b0 + batch]
+        qs, k2s, k1s = ([info[p][j] for p in pb] for j in range(3))
+        V = torch.from_numpy(np.stack([dense[p % nk1][p // nk1] for p in pb])).cuda()
+        T = blk.transform(V, qs, k2s, k1s)
+        trip += blk.triples_from_maxabs(blk.block_maxabs(T, qs, k2s, k1s), qs, k2s, k1s, 1e-9, vmax)
+        Ts.append((T.cpu(), qs, k2s, k1s))
+    tptr = np.zeros(cfg.npairs + 1, np.int64)
+    tptr[1:] = np.cumsum([len(t) for t in trip])
+    lib.set_triples(tptr, np.concatenate(trip))
+    cfg.triple_ptr, cfg.triples = tptr, trip
+    total = lib.buffer_sizes()[3]
+    out = torch.zeros(total, dtype=torch.complex128, device="cuda")
+    base = 0
+    for bi, (T, qs, k2s, k1s) in enumerate(Ts):
+        tabs = blk.pack_tables(trip[bi * batch:bi * batch + len(qs)], qs, k2s, k1s)
+        off = np.concatenate([[0], np.cumsum(tabs[3])])
+        blk.pack(T.cuda(), qs, k2s, k1s, tabs, out, off[:-1] + base)
+        base += int(off[-1])
+    assert base == total
+    return out.cpu().numpy()
+
+
 def _sampled(name, mode, pick, taus, pushes_q=None):
     """BASELINE configs too large for a full oracle run: Sigma at a few wedge points (every output k1 is an
     independent sum over all q, gwsig_set_output_points), all tau on the GPU, oracle at the sampled tau."""
@@ -134,7 +175,7 @@ def _sampled(name, mode, pick, taus, pushes_q=None):
     lib = B.Gwsig(device=0)
     cfg = configure_from_crystal(lib, inp.cr, mode, out_points=pick)
     G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
-    V = cfg.pack_V(inp.V2_rows)
+    V = _pack_V_device(cfg, inp) if (mode == 2 and name in ("cfg4", "cfg5")) else cfg.pack_V(inp.V2_rows)
     sig = run_gpu(cfg, G, W, V, pushes=None if pushes_q is None else pushes_q * cfg.nk1)
     w = _check(cfg, inp, sig, ks=[int(k) for k in cfg.out_list], taus=taus)
     print(name, "mode", mode, "points", list(cfg.out_list), "tau", list(taus), "worst rel err", w)
