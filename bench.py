@@ -46,6 +46,7 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--mode", default="ibz_block", choices=list(MODES))
     ap.add_argument("--no-modes", action="store_true", help="skip the FULL_BZ / IBZ comparison legs")
+    ap.add_argument("--no-cfg4", action="store_true", help="default workload only: skip the cfg4 sub-record (1 warm-up + 1 step, ~3 min)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--cpu-sample-tau", type=int, default=4, help="tau points of the oracle sample")
@@ -602,6 +603,31 @@ def main():
             for m in modes.values():
                 m["speedup_vs_full_bz"] = base / m["ms"]
         line["modes"] = modes
+
+    # ---- the other target config of the north star (configs 3-4): one step of cfg4 in the same job ------------------------------
+    if args.workload == "cfg3" and not args.no_cfg4 and world == 1:
+        wl.V = None
+        dG = dW = dS = None
+        torch.cuda.empty_cache()
+        t4 = time.time()
+        w4 = Workload("cfg4", MODES[args.mode], B, pack, torch=torch, dev=dev, device_index=local)
+        w4.lib.set_option("engine", args.engine)
+        tt, k4, l4, dS4 = run_steps(w4, torch, dev, 1, 1, timing=True)
+        sf4 = stage_flops(w4, B)
+        ts4 = [k4[k][0] * 1e-3 for k in ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")]
+        rec = {"workload": describe("cfg4"), "mode": args.mode, "steps": 1, "warmup": 1, "ms": tt[0] * 1e3,
+               "gflops_executed": w4.executed / tt[0] / 1e9, "gflops_full_bz_equivalent": w4.full_equiv / tt[0] / 1e9,
+               "kernels_ms": {k: round(v[0], 2) for k, v in k4.items()}, "gpu_launches": int(l4),
+               "contraction": {"tflops": sum(sf4) / max(sum(ts4), 1e-12) / 1e12, "frac_fp64_tensor_peak": sum(sf4) / max(sum(ts4), 1e-12) / 1e12 / peak,
+                               "stage_tflops": [f / max(t, 1e-12) / 1e12 for f, t in zip(sf4, ts4)]},
+               **w4.setup_notes}
+        if not args.no_cpu_baseline:
+            ks4, taus4 = sample_points(list(w4.cfg.ir_list), w4.cfg.ntau, 1, 2)
+            dt4, ref4, _ = oracle_sample(w4.inp, ks4, taus4)
+            rec["parity_sample_max_rel_err"] = fold_and_compare(w4, dS4.cpu().numpy(), ref4, ks4, taus4)
+            rec["parity_sample"] = f"k={ks4}, tau idx={taus4}, oracle {dt4:.1f} s"
+        rec["wall_s"] = round(time.time() - t4, 1)
+        line["cfg4"] = rec
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

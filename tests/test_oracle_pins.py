@@ -257,3 +257,68 @@ def test_exchange_gauge_covariance_and_hermiticity():
                       lambda a, b: np.einsum("ip,Qpq,jq->Qij", T[a], inp.V_pair(a, b), T[b].conj()), ks)
     for k in ks:
         assert np.abs(K2[k] - T[k] @ K[k] @ T[k].conj().T).max() < 1e-13 * np.abs(K).max()
+
+
+# ---- bare bubble P0, Eq. 20 / Algorithm 3 --------------------------------
+def _kadd(inp):
+    return lambda k, q: int(inp.kmesh.index(inp.kmesh.n[k] + inp.kmesh.n[q]))
+
+
+def test_p0_brute_vs_ref_and_einsum():
+    from oracle.p0_oracle import p0_brute, p0_ref
+    inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=2, naux=3, ntau=3, beta=3.0, nocc=1, seed=8)
+    rng = np.random.default_rng(4)
+    G = rng.standard_normal((inp.nk, 3, 2, 2)) + 1j * rng.standard_normal((inp.nk, 3, 2, 2))       # no structure assumed
+    V = {(a, b): rng.standard_normal((3, 2, 2)) + 1j * rng.standard_normal((3, 2, 2)) for a in range(inp.nk) for b in range(inp.nk)}
+    add = _kadd(inp)
+    qs = [0, 3]
+    brute = p0_brute(inp.nk, add, G, lambda a, b: V[(a, b)], qs)
+    ref = p0_ref(inp.nk, add, lambda k: G[k], lambda a, b: V[(a, b)], qs)
+    assert np.abs(brute - ref).max() < 1e-13 * np.abs(ref).max()
+    for iq, q in enumerate(qs):
+        for n in range(3):
+            want = -sum(np.einsum("Qda,cd,ab,Pbc->QP", V[(k, add(k, q))], -G[k, 2 - n], G[add(k, q), n], V[(add(k, q), k)])
+                        for k in range(inp.nk)) / inp.nk
+            assert np.abs(ref[iq, n] - want).max() < 1e-13 * np.abs(want).max()
+    sub = p0_ref(inp.nk, add, lambda k: G[k], lambda a, b: V[(a, b)], qs, tau_idx=[2, 0])
+    assert np.abs(sub - ref[:, [2, 0]]).max() == 0
+
+
+def test_p0_single_level_closed_form():
+    """one orbital, one auxiliary function, a k-independent level eps and coupling v: P0 = |v|^2 n_F (1 - n_F) for every tau
+    (G(tau) = -e^{-eps tau}/(1 + e^{-beta eps}); -G(-tau) G(tau) = G(beta - tau) G(tau) = e^{-beta eps}/(1 + e^{-beta eps})^2)."""
+    from oracle.p0_oracle import p0_ref
+    beta, eps, v, ntau, nk = 4.0, 0.37, 0.8 - 0.3j, 7, 4
+    tau = np.arange(ntau) * beta / (ntau - 1)
+    g = (-np.exp(-eps * tau) / (1 + np.exp(-beta * eps))).reshape(ntau, 1, 1).astype(complex)
+    P0 = p0_ref(nk, lambda k, q: (k + q) % nk, lambda k: g, lambda a, b: np.array([[[v]]]) if a <= b else np.array([[[np.conj(v)]]]), [0, 1])
+    nF = 1 / (1 + np.exp(beta * eps))
+    # q = 0: V^{k,k} V^{k,k} = v v; q = 1: pairs (k, k+1): v conj(v) except the wrap-around pair (3, 0): conj(v) v
+    assert np.abs(P0[0, :, 0, 0] - v * v * nF * (1 - nF)).max() < 1e-15
+    assert np.abs(P0[1, :, 0, 0] - abs(v) ** 2 * nF * (1 - nF)).max() < 1e-15
+
+
+def test_p0_gauge_and_hermiticity():
+    from oracle.p0_oracle import p0_ref
+    inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=4, ntau=4, beta=3.0, nocc=1, seed=6)
+    G = inp.G_full()
+    add = _kadd(inp)
+    qs = list(range(inp.nk))
+    P0 = p0_ref(inp.nk, add, lambda k: G[k], inp.V_pair, qs)
+    assert np.abs(P0 - P0.conj().transpose(0, 1, 3, 2)).max() < 1e-13 * np.abs(P0).max()      # G Hermitian, V^{k'k} = V^{kk'}^dagger
+    rng = np.random.default_rng(2)
+    T = [np.linalg.qr(rng.standard_normal((3, 3)) + 1j * rng.standard_normal((3, 3)))[0] for _ in range(inp.nk)]
+    P0g = p0_ref(inp.nk, add, lambda k: T[k] @ G[k] @ T[k].conj().T,
+                 lambda a, b: np.einsum("ip,Ppq,jq->Pij", T[a], inp.V_pair(a, b), T[b].conj()), qs)
+    assert np.abs(P0g - P0).max() < 1e-13 * np.abs(P0).max()                                  # orbital gauge: invariant
+    # auxiliary gauge S at momentum q: V^{k,k+q}(Q) -> S V, its partner V^{k+q,k} = (V^{k,k+q})^dagger -> conj(S) V: P0 -> S P0 S^dagger
+    S = np.linalg.qr(rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4)))[0]
+    q = 3
+    calls = {"n": 0}
+
+    def Vaux(a, b):
+        calls["n"] += 1                      # p0_ref asks for V^{k,k+q} first, V^{k+q,k} second
+        return np.einsum("PQ,Qij->Pij", S if calls["n"] % 2 == 1 else S.conj(), inp.V_pair(a, b))
+    P0s = p0_ref(inp.nk, add, lambda k: G[k], Vaux, [q])[0]
+    want = np.einsum("PQ,tQR,SR->tPS", S, P0[q], S.conj())
+    assert np.abs(P0s - want).max() < 1e-13 * np.abs(P0).max()
