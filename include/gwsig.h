@@ -175,6 +175,23 @@ int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, co
 int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream);
 int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream);
 
+/* ---- N1: bare bubble ---------------------------------------------------------------
+ * P0^q_{QQ'}(tau) = -(1/Nk) sum_k sum_{abcd} V^{k,k+q}_{Q,da} G^k_{cd}(-tau) G^{k+q}_{ab}(tau) V^{k+q,k}_{Q',bc}   (Eq. 20,
+ * PAPER.md:179-184; one spin channel) in the order of Algorithm 3: X1 = V G^k(-tau), X2 = V G^{k+q}(tau),
+ * P0 += X1 X2, for every q of the output list (the wedge in GWSIG_IBZ mode -- "Eq. 20 is evaluated for q in IBZ",
+ * every mesh point in GWSIG_FULL_BZ; GWSIG_IBZ_BLOCK is refused) and every tau of the grid, which must be
+ * uniform on [0, beta]: G(-tau_n) = -G(beta - tau_n) = -G[ntau-1-n].
+ *   dG   : as for sigma_begin (wedge data in IBZ mode, unfolded by Eq. 22)
+ *   dV   : T = V^{k,k+q}_{Q,da} as [naux][nao][nao] per pair, pairs ordered k-major: pair = k * nq + iq, q = q_list[iq]
+ *          (gwsig_get_ibz / set_output_points give the list), k over the whole mesh; the partner V^{k+q,k} is taken as the
+ *          conjugate transpose (reading A7 of DESIGN.md)
+ *   dP0  : [nq][ntau][naux][naux], written by p0_end
+ * p0_push_pairs takes ranges in increasing order without gaps, like sigma_push_pairs; p0_eval = begin + one push + end.  */
+int gwsig_p0_begin(gwsig_ctx* ctx, const void* dG, void* dP0, void* stream);
+int gwsig_p0_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV);
+int gwsig_p0_end(gwsig_ctx* ctx);
+int gwsig_p0_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, void* dP0, void* stream);
+
 /* ---- options and accounting ------------------------------------------------------------------ */
 /* keys: "engine" (gwsig_engine), "hermitize" (0/1, default 0), "scratch_mib" (X+Y scratch budget,
  * default 8192), "tau_chunk" (0 = from the budget), "v_ring_mib" (size of one slot of the
@@ -199,7 +216,8 @@ int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
 int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
- * stage: 1 = X = V G lowered transposed, X^T = G^T conj(V2) (A = G, B = V2, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
+ * stage: 31, 32, 33 = the three stages of the bare bubble (p0 / np then count P0 pairs); 11, 12 / 21, 22 = the two launches of
+ * the Eq. 28 block unfold of G / W (p0 = first mesh point, np = number of points); 1 = X = V G lowered transposed, X^T = G^T conj(V2) (A = G, B = V2, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
  * B = W, C = Y), 3 = Sigma += Y V (A = Y, B = V2, C = Sigma accumulator; the segment list of an
  * output block may be cut into several problems that add into the same C).
  * Descriptors are the structs of include/gwsig_plan.h; offsets are in complex elements relative

@@ -35,7 +35,8 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_pair_info", "gwsig_buffer_sizes", "gwsig_sigma_begin", "gwsig_sigma_push_pairs", "gwsig_sigma_end",
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
            "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host",
-           "gwsig_set_output_points", "gwsig_exchange_begin", "gwsig_exchange_eval"]
+           "gwsig_set_output_points", "gwsig_exchange_begin", "gwsig_exchange_eval",
+           "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -52,6 +53,8 @@ _sig = {
     "gwsig_probe_fp64": [_vp, _i, _i, _i, _i64, _vp, _vp], "gwsig_kernel_times": [_vp, _vp, _vp],
     "gwsig_sigma_abort": [_vp], "gwsig_sigma_eval_host": [_vp, _vp, _vp, _vp, _vp, _vp],
     "gwsig_exchange_begin": [_vp, _vp, _vp, _vp], "gwsig_exchange_eval": [_vp, _vp, _vp, _vp, _vp],
+    "gwsig_p0_begin": [_vp, _vp, _vp, _vp], "gwsig_p0_push_pairs": [_vp, _i64, _i64, _vp], "gwsig_p0_end": [_vp],
+    "gwsig_p0_eval": [_vp, _vp, _vp, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -217,6 +220,18 @@ class Gwsig:
 
     def exchange_eval(self, dGamma, dV, dK, stream=0):
         self._ck(_lib.gwsig_exchange_eval(self._h, _ptr(dGamma), _ptr(dV), _ptr(dK), stream or None))
+
+    def p0_begin(self, dG, dP0, stream=0):
+        self._ck(_lib.gwsig_p0_begin(self._h, _ptr(dG), _ptr(dP0), stream or None))
+
+    def p0_push_pairs(self, p0, np_, dV):
+        self._ck(_lib.gwsig_p0_push_pairs(self._h, p0, np_, _ptr(dV)))
+
+    def p0_end(self):
+        self._ck(_lib.gwsig_p0_end(self._h))
+
+    def p0_eval(self, dG, dV, dP0, stream=0):
+        self._ck(_lib.gwsig_p0_eval(self._h, _ptr(dG), _ptr(dV), _ptr(dP0), stream or None))
 
     def sigma_abort(self):
         self._ck(_lib.gwsig_sigma_abort(self._h))

@@ -74,7 +74,11 @@ struct gwsig_ctx {
   long long launches = 0;
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
-  DevBuf oblk_ao, oblk_aux, unf_tmp, partial;    // partial: split-K partial tiles of deterministic stage 3
+  DevBuf oblk_ao, oblk_aux, unf_tmp, partial;
+  DevBuf grev, p0acc, p0desc;                    // N1 (Eq. 20): G(beta - tau) on the full zone, the P0 accumulator, its epilogue descriptors
+  bool in_p0 = false;
+  double2* dP0 = nullptr;
+  std::map<std::tuple<long long, long long, int>, std::unique_ptr<DevPlan>> p0_cache;    // partial: split-K partial tiles of deterministic stage 3
   DevBuf __unused_;             // Eq. 28: O_block tables and the scratch T of the two-step block unfold
   DevBuf h_g, h_w, h_sig, h_vslot[2];           // device side of sigma_eval_host
   cudaStream_t copy_stream = nullptr;
@@ -347,7 +351,11 @@ static void invalidate(gwsig_ctx* ctx) {
   for (auto& kv : ctx->plan_cache)
     for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); kv.second->st[s].red.release(); }
   ctx->plan_cache.clear();
+  for (auto& kv : ctx->p0_cache)
+    for (int s = 0; s < 3; ++s) { kv.second->st[s].prob.release(); kv.second->st[s].seg.release(); kv.second->st[s].bucket.release(); }
+  ctx->p0_cache.clear();
   ctx->in_eval = false;
+  ctx->in_p0 = false;
 }
 
 // =============================================================================================
@@ -366,7 +374,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -533,9 +541,10 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
                       int64_t* ntiles) {
   if (!ctx) return GWSIG_ERR_ARG;
   const Plan& P = ctx->plan;
-  if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
+  if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
+  int rc = stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
+         : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_counts: bad range / stage");
   if (nproblems) *nproblems = (int64_t)sp.prob.size();
@@ -547,9 +556,10 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
 int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, void* problems_out, void* segs_out) {
   if (!ctx || !problems_out || !segs_out) return GWSIG_ERR_ARG;
   const Plan& P = ctx->plan;
-  if (!P.have_sym || P.v_off.empty()) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
+  if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
+  int rc = stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
+         : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_get: bad range / stage");
   std::memcpy(problems_out, sp.prob.data(), sp.prob.size() * sizeof(gwsig_problem));
@@ -753,6 +763,128 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
   rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
   if (rc) { ctx->in_eval = false; ctx->exchange = false; return rc; }
   return gwsig_sigma_end(ctx);
+}
+
+/* ---- N1: bare bubble P0^q(tau) (Eq. 20, Algorithm 3), dense modes ---------------------------- */
+int gwsig_p0_begin(gwsig_ctx* ctx, const void* dG, void* dP0, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "p0_begin: call set_symmetry first");
+  if (P.mode == GWSIG_IBZ_BLOCK) return fail(ctx, GWSIG_ERR_ARG, "p0_begin: the bare bubble is built for the dense modes (FULL_BZ, IBZ) only");
+  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "p0_begin: an evaluation is already open");
+  if (!dG || !dP0) return fail(ctx, GWSIG_ERR_ARG, "p0_begin: NULL device pointer");
+  // reuse sigma_begin for the device set-up and the unfold of G (Eq. 22); it needs no W for that
+  ctx->exchange = true;
+  int rc = gwsig_sigma_begin(ctx, dG, nullptr, dP0, stream);
+  ctx->exchange = false;
+  ctx->in_eval = false;
+  if (rc) return rc;
+  const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
+  const long long n2 = (long long)P.nao * P.nao;
+  CU(ctx->grev.ensure((size_t)P.nk * P.ntau * n2 * sizeof(double2)));
+  // G(-tau_n) = -G(beta - tau_n) = -G[ntau-1-n] (fermionic antiperiodicity, uniform grid): the reversed copy; the sign goes
+  // into the epilogue (-(1/Nk) of Eq. 20 becomes +1/Nk)
+  CU(launch_reverse_tau(Gsrc, (double2*)ctx->grev.p, P.nk, P.ntau, n2, ctx->stream));
+  ctx->launches++;
+  const size_t pe = (size_t)P.nk1 * P.ntau * P.naux * P.naux;
+  CU(ctx->p0acc.ensure(std::max<size_t>(pe * sizeof(double2), 16)));
+  CU(cudaMemsetAsync(ctx->p0acc.p, 0, pe * sizeof(double2), ctx->stream));
+  ctx->dP0 = (double2*)dP0;
+  ctx->next_pair = 0;
+  ctx->in_p0 = true;
+  return GWSIG_OK;
+}
+
+int gwsig_p0_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "p0_push_pairs: call p0_begin first");
+  const long long npairs = (long long)P.nk * P.nk1;
+  if (np < 1 || p0 != ctx->next_pair || p0 + np > npairs)
+    return fail(ctx, GWSIG_ERR_ORDER, "p0_push_pairs: ranges must be pushed in increasing order without gaps");
+  if (!dV) return fail(ctx, GWSIG_ERR_ARG, "p0_push_pairs: NULL device pointer");
+  CU(cudaSetDevice(ctx->device));
+  const long long xs = (long long)P.naux * P.nao * P.nao;
+  size_t free_b = 0, total_b = 0;
+  CU(cudaMemGetInfo(&free_b, &total_b));
+  const double avail = 0.4 * ((double)free_b + (double)ctx->xbuf.bytes + (double)ctx->ybuf.bytes);
+  const double budget = std::min((double)ctx->scratch_mib * 1048576.0, std::max(avail, 64.0 * 1048576.0)) / (2.0 * sizeof(double2));
+  const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
+  const double2* Vbase = (const double2*)dV;
+  long long s0 = p0;
+  while (s0 < p0 + np) {
+    // sub-batch: as many pairs as fit the X1 / X2 scratch for at least one tau; then as many tau as fit
+    long long ns = std::max<long long>(1, std::min<long long>(p0 + np - s0, (long long)(budget / (double)xs)));
+    int nt_max = ctx->tau_chunk > 0 ? ctx->tau_chunk : (int)std::max(1.0, std::floor(budget / ((double)xs * (double)ns)));
+    nt_max = std::min(nt_max, P.ntau);
+    const int nchunks = (P.ntau + nt_max - 1) / nt_max;
+    const int nt = (P.ntau + nchunks - 1) / nchunks;
+    const size_t xbytes = (size_t)xs * ns * nt * sizeof(double2);
+    CU(ctx->xbuf.ensure(xbytes));
+    CU(ctx->ybuf.ensure(xbytes));
+    const double2* Vsub = Vbase + (s0 - p0) * xs;
+    for (int t0 = 0; t0 < P.ntau; t0 += nt) {
+      const int ntc = std::min(nt, P.ntau - t0);
+      auto key = std::make_tuple((long long)s0, (long long)ns, ntc);
+      DevPlan* dp = nullptr;
+      auto it = ctx->p0_cache.find(key);
+      if (it != ctx->p0_cache.end()) dp = it->second.get();
+      else {
+        std::unique_ptr<DevPlan> np_(new DevPlan());
+        for (int s = 0; s < 3; ++s) {
+          StagePlan sp;
+          int rc = P.build_p0_stage(s0, ns, ntc, s + 1, sp, ctx->num_sms > 0 ? ctx->num_sms : 148);
+          if (rc) return fail(ctx, rc, "internal: build_p0_stage failed");
+          DevStage& d = np_->st[s];
+          d.nprob = (int)sp.prob.size(); d.ntiles = sp.ntiles;
+          if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
+          if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
+          if ((rc = upload(ctx, d.bucket, sp.bucket))) return rc;
+        }
+        dp = np_.get();
+        ctx->p0_cache[key] = std::move(np_);
+      }
+      int rc;
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], (const double2*)ctx->grev.p, Vsub, (double2*)ctx->xbuf.p, t0))) return rc;   // X1
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], Gsrc, Vsub, (double2*)ctx->ybuf.p, t0))) return rc;                          // X2
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->xbuf.p, (const double2*)ctx->ybuf.p, (double2*)ctx->p0acc.p, t0))) return rc;
+    }
+    s0 += ns;
+  }
+  ctx->next_pair = p0 + np;
+  return GWSIG_OK;
+}
+
+int gwsig_p0_end(gwsig_ctx* ctx) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "p0_end: call p0_begin first");
+  if (ctx->next_pair != (long long)P.nk * P.nk1) return fail(ctx, GWSIG_ERR_ORDER, "p0_end: not all pairs were pushed");
+  CU(cudaSetDevice(ctx->device));
+  std::vector<EpiDesc> ed;
+  for (int iq = 0; iq < P.nk1; ++iq) ed.push_back(EpiDesc{(long long)iq * P.ntau * P.naux * P.naux, (long long)P.naux * P.naux, P.naux, P.ntau});
+  int rc = upload(ctx, ctx->p0desc, ed);
+  if (rc) return rc;
+  EpilogueParams ep;
+  ep.acc = (const double2*)ctx->p0acc.p;
+  ep.out = ctx->dP0;
+  ep.desc = (const EpiDesc*)ctx->p0desc.p;
+  ep.scale = 1.0 / (double)P.nk;          // -(1/Nk) of Eq. 20 times the -1 of G(-tau) = -G(beta - tau)
+  ep.hermitize = ctx->hermitize;
+  if ((rc = tic(ctx, GWSIG_KIND_EPILOGUE))) return rc;
+  CU(launch_epilogue(ep, (int)ed.size(), ctx->num_sms, ctx->stream));
+  if ((rc = toc(ctx))) return rc;
+  ctx->launches++;
+  ctx->in_p0 = false;
+  return GWSIG_OK;
+}
+
+int gwsig_p0_eval(gwsig_ctx* ctx, const void* dG, const void* dV_all, void* dP0, void* stream) {
+  int rc = gwsig_p0_begin(ctx, dG, dP0, stream);
+  if (rc) return rc;
+  rc = gwsig_p0_push_pairs(ctx, 0, (int64_t)ctx->plan.nk * ctx->plan.nk1, dV_all);
+  if (rc) { ctx->in_p0 = false; return rc; }
+  return gwsig_p0_end(ctx);
 }
 
 int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, const void* hW, void* hSigma, void* stream) {

@@ -266,6 +266,20 @@ cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_
   return cudaGetLastError();
 }
 
+__global__ void __launch_bounds__(256) reverse_tau_kernel(const double2* src, double2* dst, int ntau, long long elems) {
+  const long long kt = blockIdx.x;                       // k * ntau + n   (grid.x: Nk * ntau exceeds 65535 at config 5)
+  const long long k = kt / ntau, n = kt % ntau;
+  const double2* s_ = src + (k * ntau + (ntau - 1 - n)) * elems;
+  double2* d_ = dst + kt * elems;
+  for (long long e = threadIdx.x; e < elems; e += blockDim.x) d_[e] = s_[e];
+}
+
+cudaError_t launch_reverse_tau(const double2* src, double2* dst, int nk, int ntau, long long elems, cudaStream_t stream) {
+  if (nk <= 0 || ntau <= 0) return cudaSuccess;
+  reverse_tau_kernel<<<(unsigned)((long long)nk * ntau), 256, 0, stream>>>(src, dst, ntau, elems);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream) {
   if (ngroups <= 0) return cudaSuccess;
   for (int g0 = 0; g0 < ngroups; g0 += 65535) {

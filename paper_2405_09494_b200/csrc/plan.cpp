@@ -26,6 +26,13 @@ int Plan::ksub(int k, int q) const {
   return kindex(a_[0] - b_[0], a_[1] - b_[1], a_[2] - b_[2]);
 }
 
+int Plan::kadd(int k, int q) const {
+  int a_[3], b_[3];
+  kcoords(k, a_);
+  kcoords(q, b_);
+  return kindex(a_[0] + b_[0], a_[1] + b_[1], a_[2] + b_[2]);
+}
+
 int Plan::set_lattice(const double a_[9], const int mesh[3], int nao_, int naux_, int ntau_, double beta_) {
   if (!a_ || !mesh) { err = "set_lattice: NULL argument"; return GWSIG_ERR_ARG; }
   if (mesh[0] < 1 || mesh[1] < 1 || mesh[2] < 1 || nao_ < 1 || naux_ < 1 || ntau_ < 1) {
@@ -701,6 +708,109 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
   }
+  out.ntiles = tb;
+  out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
+  size_t pi = 0;
+  for (size_t bkt = 0; bkt < out.bucket.size(); ++bkt) {
+    const long long t = (long long)bkt << ZG_BUCKET_SHIFT;
+    while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
+    out.bucket[bkt] = (int)pi;
+  }
+  return GWSIG_OK;
+}
+
+int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePlan& out, int num_sms) const {
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
+  if (mode == GWSIG_IBZ_BLOCK) return GWSIG_ERR_ARG;                // dense modes only
+  if (p0 < 0 || np < 1 || p0 + np > (long long)nk * nk1 || nt < 1 || nt > ntau || stage < 1 || stage > 3) return GWSIG_ERR_ARG;
+  const long long n2 = (long long)nao * nao, xs = (long long)naux * n2, gts = n2, wts = (long long)naux * naux;
+  std::vector<long long> cost;
+  if (stage == 1 || stage == 2) {
+    for (long long l = 0; l < np; ++l) {
+      int k, q, kq, iq;
+      p0_pair(p0 + l, k, q, kq, iq);
+      gwsig_seg S; std::memset(&S, 0, sizeof(S));
+      gwsig_problem P; std::memset(&P, 0, sizeof(P));
+      S.K = nao;
+      P.M = nt * nao; P.N = naux * nao;
+      P.c_off = l * xs * nt;
+      P.a_tstride = gts;
+      P.nbatch = 1;
+      if (stage == 1) {
+        // X1^T[(tau,c),(Q,a)] = sum_d Grev^k[(tau,c),d] T[d,(Q,a)]                    (Algorithm 3 line 6)
+        S.a_off = (long long)k * ntau * gts;
+        S.am = lvl2(nao, gts, nao); S.ak = lvl1(1);
+        S.b_off = l * xs;
+        S.bk = lvl1(nao); S.bn = lvl2(nao, n2, 1);           // n = (Q, a): T[Q][d][a]
+        P.cm = lvl2(nao, xs, (long long)nao * naux);         // X1[tau][(c,a)][Q]
+        P.cn = lvl2(nao, 1, naux);
+        P.flags = 0;
+      } else {
+        // X2^T[(tau,a),(Q',c)] = sum_b G^{kq}[(tau,a),b] conj(T[Q'][c][b])              (Algorithm 3 line 7)
+        S.a_off = (long long)kq * ntau * gts;
+        S.am = lvl2(nao, gts, nao); S.ak = lvl1(1);
+        S.b_off = l * xs;
+        S.bk = lvl1(1); S.bn = lvl2(nao, n2, nao);           // n = (Q', c): T[Q'][c][b]
+        P.cm = lvl2(nao, xs, naux);                          // X2[tau][(c,a)][Q']: a * naux
+        P.cn = lvl2(nao, 1, (long long)nao * naux);          // Q' + c * nao * naux
+        P.flags = GWSIG_FLAG_CONJ_B;
+      }
+      P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+      out.seg.push_back(S); out.prob.push_back(P); cost.push_back(S.K);
+    }
+  } else {
+    // P0acc[iq][tau][Q][Q'] += sum_pairs sum_{(c,a)} X1[(c,a)][Q] X2[(c,a)][Q']       (Algorithm 3 line 8); the pairs
+    // (k) of one q are the segments, cut into parts that add into the same block (FP64 atomics), one batch entry per tau
+    long long tiles1 = 0;
+    std::vector<std::vector<gwsig_seg>> segs(nk1);
+    for (long long l = 0; l < np; ++l) {
+      int k, q, kq, iq;
+      p0_pair(p0 + l, k, q, kq, iq);
+      gwsig_seg S; std::memset(&S, 0, sizeof(S));
+      S.a_off = l * xs * nt; S.am = lvl1(1); S.ak = lvl1(naux);       // A[m = Q, k = (c,a)] = X1[(c,a)][Q]
+      S.b_off = l * xs * nt; S.bk = lvl1(naux); S.bn = lvl1(1);       // B[k = (c,a), n = Q'] = X2[(c,a)][Q']
+      S.K = (int)n2;
+      segs[iq].push_back(S);
+    }
+    for (int iq = 0; iq < nk1; ++iq)
+      if (!segs[iq].empty()) tiles1 += (long long)nt * zg_tiles_m(naux, tile_m[3]) * zg_tiles_n(naux);
+    const long long want = 12LL * std::max(num_sms, 1);
+    for (int iq = 0; iq < nk1; ++iq) {
+      if (segs[iq].empty()) continue;
+      long long parts = tiles1 > 0 ? (want + tiles1 - 1) / tiles1 : 1;
+      parts = std::max(1LL, std::min<long long>(parts, (long long)segs[iq].size()));
+      const size_t nsg = segs[iq].size();
+      for (long long part = 0; part < parts; ++part) {
+        const size_t s0 = nsg * part / parts, s1 = nsg * (part + 1) / parts;
+        if (s1 <= s0) continue;
+        gwsig_problem P; std::memset(&P, 0, sizeof(P));
+        P.M = naux; P.N = naux;
+        P.c_off = (long long)iq * ntau * wts;
+        P.cm = lvl1(naux); P.cn = lvl1(1);
+        P.a_bstride = xs; P.b_bstride = xs; P.c_bstride = wts; P.c_tstride = wts;
+        P.nbatch = nt;
+        P.flags = GWSIG_FLAG_ACCUM;
+        P.seg_begin = (int)out.seg.size();
+        for (size_t s_ = s0; s_ < s1; ++s_) out.seg.push_back(segs[iq][s_]);
+        P.seg_count = (int)(s1 - s0);
+        out.prob.push_back(P); cost.push_back((long long)(s1 - s0) * n2);
+      }
+    }
+  }
+  std::vector<int> order(out.prob.size());
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost[x] > cost[y]; });
+  std::vector<gwsig_problem> sorted(out.prob.size());
+  long long tb = 0;
+  for (size_t i = 0; i < order.size(); ++i) {
+    gwsig_problem P = out.prob[order[i]];
+    P.tiles_m = zg_tiles_m(P.M, tile_m[stage]);
+    P.tiles_n = zg_tiles_n(P.N);
+    P.tile_begin = tb;
+    tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
+    sorted[i] = P;
+  }
+  out.prob.swap(sorted);
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;

@@ -127,6 +127,18 @@ struct Plan {
   long long unfolded_elems(bool aux, int k_first, int k_count) const;
   int compute_oblock(bool aux);
   void flop_counts(double& full_equiv, double& executed) const;
+
+  // ---- N1: bare bubble P0^q(tau), Eq. 20 / Algorithm 3, dense modes -------------------------
+  // pairs are k-major: pair = k * nk1 + iq, q = out_list[iq] (the wedge in the IBZ mode), kq = k + q; the caller supplies
+  // T = V^{k,k+q}_{Q,da} [naux][nao][nao] per pair (its partner V^{k+q,k} is the conjugate transpose, reading A7)
+  int kadd(int k, int q) const;
+  void p0_pair(long long p, int& k, int& q, int& kq, int& iq) const {
+    k = (int)(p / nk1); iq = (int)(p % nk1); q = out_list[iq]; kq = kadd(k, q);
+  }
+  // stage 1: X1[(c,a)][Q] = sum_d Grev^k[c,d] T[Q,d,a]   (Grev(tau_n) = G(beta - tau_n): G(-tau) = -Grev, sign in the epilogue)
+  // stage 2: X2[(c,a)][Q'] = sum_b G^{kq}[a,b] conj(T[Q',c,b])
+  // stage 3: P0acc[iq][tau][Q][Q'] += sum over the pairs of the range with that q, sum_{(c,a)} X1[(c,a)][Q] X2[(c,a)][Q']
+  int build_p0_stage(long long p0, long long np, int nt, int stage, StagePlan& out, int num_sms = 148) const;
 };
 
 static inline long long sumsq(const std::vector<int>& off) {

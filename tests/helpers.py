@@ -228,3 +228,70 @@ def unfold_blocks_numpy(lib, stage0, k_first, k_count, X_flat, O_list, ntau):
     out = np.zeros(n_out, complex)
     run_stage_numpy(pr2, sg2, T, Opad, out, 0)
     return out
+
+
+# ---- N1: bare bubble (Eq. 20) ---------------------------------------------------------------------------------
+def p0_pairs(cfg, inp):
+    """(k, q, k+q) of every P0 pair in the library's order: pair = k * nq + iq, q = out_list[iq]."""
+    km = inp.kmesh
+    return [(k, int(q), int(km.index(km.n[k] + km.n[int(q)]))) for k in range(cfg.nk) for q in cfg.out_list]
+
+
+def pack_V_p0(cfg, inp):
+    """T = V^{k,k+q}_{Q,da} [naux][nao][nao] for every P0 pair, flat."""
+    return np.ascontiguousarray(np.concatenate([inp.V_pair(k, kq).ravel() for (k, q, kq) in p0_pairs(cfg, inp)]), np.complex128)
+
+
+def oracle_p0(inp, qs, taus=None):
+    """oracle/p0_oracle.p0_ref with independently generated V^{k,k+q} (V_pair(k, k+q)) and V^{k+q,k} (V_pair(k+q, k))."""
+    from oracle.p0_oracle import p0_ref
+    km = inp.kmesh
+    Gc = {}
+
+    def G_of(k):
+        if k not in Gc:
+            Gc[k] = inp.G_k(k) if hasattr(inp, "G_k") else inp.G_full()[k]
+        return Gc[k]
+    return p0_ref(inp.nk, lambda k, q: int(km.index(km.n[k] + km.n[q])), G_of, inp.V_pair, [int(q) for q in qs], taus)
+
+
+def run_p0_plan_numpy(cfg, inp, G_flat, V_flat, push_pairs=None, nt=None):
+    """emulate gwsig_p0_eval with the descriptors of plan stages 31, 32, 33 (Algorithm 3) -> [nq, ntau, naux, naux]."""
+    lib = cfg.lib
+    ntau, nao, naux, nk = cfg.ntau, cfg.nao, cfg.naux, cfg.nk
+    nq = len(cfg.out_list)
+    npairs = nk * nq
+    nt = ntau if nt is None else nt
+    push_pairs = npairs if push_pairs is None else push_pairs
+    if cfg.mode == IBZ:
+        cr = inp.cr
+        Gi = G_flat.reshape(len(cfg.ir_list), ntau, nao, nao)
+        ir_index = {int(k): i for i, k in enumerate(cfg.ir_list)}
+        Gs = []
+        for k in range(nk):
+            g = int(cfg.op_of[k])
+            O = rep_at_k(cr.P_ao[g], cr.ao_atom, cr.sg.shift[g], cr.kmesh.frac[k])
+            Gs.append(O @ Gi[ir_index[int(cfg.ir_of[k])]] @ O.conj().T)
+        Gsrc = np.stack(Gs)
+    else:
+        Gsrc = G_flat.reshape(nk, ntau, nao, nao)
+    Grev = np.ascontiguousarray(Gsrc[:, ::-1]).ravel()          # G(beta - tau); the sign of G(-tau) = -G(beta - tau) is in the scale
+    Gsrc = np.ascontiguousarray(Gsrc).ravel()
+    acc = np.zeros(nq * ntau * naux * naux, complex)
+    xs = naux * nao * nao
+    p0 = 0
+    while p0 < npairs:
+        npp = min(push_pairs, npairs - p0)
+        Vsub = V_flat[p0 * xs:(p0 + npp) * xs]
+        for t0 in range(0, ntau, nt):
+            ntc = min(nt, ntau - t0)
+            X1 = np.zeros(npp * xs * ntc, complex)
+            X2 = np.zeros(npp * xs * ntc, complex)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 31)
+            run_stage_numpy(pr, sg, Grev, Vsub, X1, t0)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 32)
+            run_stage_numpy(pr, sg, Gsrc, Vsub, X2, t0)
+            pr, sg, _ = lib.plan_get(p0, npp, ntc, 33)
+            run_stage_numpy(pr, sg, X1, X2, acc, t0)
+        p0 += npp
+    return (acc / nk).reshape(nq, ntau, naux, naux)

@@ -4,7 +4,7 @@ FP64, after folding the result back to the orbital basis."""
 import numpy as np
 import pytest
 
-from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_sigma, rel_err
+from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_p0, oracle_sigma, pack_V_p0, rel_err
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -280,6 +280,48 @@ def test_deterministic_accumulation_is_bit_reproducible():
     _check(cfg, inp, a)
     c = run_gpu(cfg, G, W, V, deterministic=0, tau_chunk=2)
     assert np.abs(a - c).max() <= 1e-12 * np.abs(a).max()
+
+
+@pytest.mark.parametrize("name,mode", [("cfg1", 0), ("toy_diamond4", 1), ("toy_wurtzite", 1), ("cfg2", 1)])
+def test_p0_eq20(name, mode):
+    """N1: bare bubble P0^q(tau) (Eq. 20, Algorithm 3) through gwsig_p0_eval / p0_push_pairs against
+    oracle/p0_oracle.py: every output q (the wedge in IBZ mode), every tau; one call, and several pushes with tau chunks."""
+    B = _B()
+    torch = _torch()
+    from paper_2405_09494_b200.pack import Configured, configure_from_crystal
+    lib = B.Gwsig(device=0)
+    if name == "cfg1":
+        inp = get_inputs("cfg1")
+        cfg = Configured(lib, mode, np.eye(3), inp.kmesh.N, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
+        Gf = inp.G_full()
+        G, _ = cfg.pack_GW(lambda k: Gf[k], lambda q: np.zeros((inp.ntau, inp.naux, inp.naux), complex))
+    else:
+        inp = get_inputs(name)
+        cfg = configure_from_crystal(lib, inp.cr, mode)
+        G, _ = cfg.pack_GW(inp.G_k, lambda q: np.zeros((inp.ntau, inp.naux, inp.naux), complex))
+    V = pack_V_p0(cfg, inp)
+    dG, dV = torch.from_numpy(G).cuda(), torch.from_numpy(V).cuda()
+    nq = len(cfg.out_list)
+    shape = (nq, inp.ntau, inp.naux, inp.naux)
+    ref = oracle_p0(inp, cfg.out_list)
+    stream = torch.cuda.current_stream().cuda_stream
+    for variant in ("eval", "pushes"):
+        dP = torch.full((int(np.prod(shape)),), float("nan"), dtype=torch.complex128, device="cuda")
+        if variant == "eval":
+            lib.set_option("tau_chunk", 0)
+            lib.p0_eval(dG, dV, dP, stream)
+        else:
+            lib.set_option("tau_chunk", max(1, inp.ntau // 3))
+            lib.p0_begin(dG, dP, stream)
+            xs = inp.naux * inp.nao ** 2
+            npairs, step = cfg.nk * nq, max(1, (cfg.nk * nq) // 3 + 1)
+            for p0 in range(0, npairs, step):
+                lib.p0_push_pairs(p0, min(step, npairs - p0), dV[p0 * xs:])
+            lib.p0_end()
+        torch.cuda.synchronize()
+        got = dP.cpu().numpy().reshape(shape)
+        worst = max(rel_err(got[i, t], ref[i, t]) for i in range(nq) for t in range(inp.ntau))
+        assert worst <= TOL, (variant, worst)
 
 
 def test_output_point_subset_matches_full_run():

@@ -208,3 +208,25 @@ def test_exchange_plan_skips_stage_two():
     got = fold_to_orbital(cfg, inp, cfg.unpack_sigma(K))
     ref = oracle_exchange(inp, gam, range(inp.nk))
     assert max(rel_err(got[k][0], ref[k]) for k in range(inp.nk)) < 1e-11
+
+
+@pytest.mark.parametrize("name,mode", [("cfg1s", B.FULL_BZ), ("toy_diamond", B.IBZ), ("toy_wurtzite", B.IBZ)])
+def test_p0_plan_matches_oracle(name, mode):
+    """N1 (Eq. 20 / Algorithm 3): the three P0 stages of the plan, run by the numpy interpreter, against oracle/p0_oracle.py:
+    every wedge q (every q in FULL_BZ), every tau, several pushes and tau chunks."""
+    from tests.helpers import oracle_p0, pack_V_p0, run_p0_plan_numpy
+    lib = B.Gwsig(device=-1)
+    if name == "cfg1s":
+        inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=5, ntau=4, beta=4.0, nocc=1, seed=2)
+        cfg = Configured(lib, mode, np.eye(3), inp.kmesh.N, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
+        Gf = inp.G_full()
+        G, _ = cfg.pack_GW(lambda k: Gf[k], lambda q: np.zeros((inp.ntau, inp.naux, inp.naux), complex))
+    else:
+        inp = make_inputs(name)
+        cfg = configure_from_crystal(lib, inp.cr, mode)
+        G, _ = cfg.pack_GW(inp.G_k, lambda q: np.zeros((inp.ntau, inp.naux, inp.naux), complex))
+    V = pack_V_p0(cfg, inp)
+    got = run_p0_plan_numpy(cfg, inp, G, V, push_pairs=5, nt=max(1, inp.ntau - 1))
+    ref = oracle_p0(inp, cfg.out_list)
+    scale = np.abs(ref).max()
+    assert np.abs(got - ref).max() < 1e-12 * scale
