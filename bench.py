@@ -144,9 +144,10 @@ class Workload:
     on demand": here it is re-derived on demand from the compact real-space table)."""
 
     def __init__(self, name, mode, B, pack, inp=None, nq_subset=None, torch=None, dev=None, device_index=0, host_only=False,
-                 resident_limit_gb=110.0, q_per_batch=None):
+                 resident_limit_gb=110.0, q_per_batch=None, dv=None):
         from gwsig_synth import make_inputs
         self.name, self.mode, self.torch, self.dev = name, mode, torch, dev
+        self.dv = dv                  # the device copy of the real-space V table is shared by the legs of a run (93 GiB at cfg5)
         self.inp = inp if inp is not None else make_inputs(name)
         inp = self.inp
         self.lib = B.Gwsig(device=-1 if host_only else device_index)
@@ -167,9 +168,8 @@ class Workload:
         if nq_ is not None and nq_ < cfg.nk:
             # FULL_BZ on a q subset: only W(q < nq) is ever read; the rest of the [Nk] buffer stays zero on the device (100 GB at cfg5)
             self.G = np.ascontiguousarray(np.stack([G_of(int(k)) for k in range(cfg.nk)]).ravel(), np.complex128)
-            Wpart = np.ascontiguousarray(np.stack([W_of(int(q)) for q in range(nq_)]).ravel(), np.complex128)
-            self.W = torch.zeros(self.lib.buffer_sizes()[1], dtype=torch.complex128, device=dev)
-            self.W[:Wpart.size] = torch.from_numpy(Wpart).to(dev)
+            # the library reads W(q) only for the q it is given pairs of: the buffer holds the first nq slices (100 GB in full at cfg5)
+            self.W = np.ascontiguousarray(np.stack([W_of(int(q)) for q in range(nq_)]).ravel(), np.complex128)
         else:
             self.G, self.W = cfg.pack_GW(G_of, W_of)
         self.nq = cfg.nk if nq_subset is None else min(nq_subset, cfg.nk)      # q slices actually pushed
@@ -194,7 +194,8 @@ class Workload:
     def _device_V(self, B, resident_limit_gb, q_per_batch):
         torch, dev, cfg, lib = self.torch, self.dev, self.cfg, self.lib
         t0 = time.time()
-        self.dv = DeviceV(self.inp, torch, dev)
+        if self.dv is None:
+            self.dv = DeviceV(self.inp, torch, dev)
         nel = self.dv.nel
         nk1 = cfg.nk1
         qb = q_per_batch or max(1, int(2.0e9 // (nk1 * nel * 16)))            # ~2 GB of dense V per generation batch
@@ -521,6 +522,8 @@ def main():
         if world > 1:
             dist.destroy_process_group()
         return
+    sys.stderr.write("[bench] main leg: %.1f ms per evaluation, kernels %s\n" % (ms_eval, {k: round(v[0], 1) for k, v in kinds.items()}))
+    sys.stderr.flush()
 
     # ---- accounting: flops, stage shares, roofline ------------------------------------------------------------
     sf = stage_flops(wl, B)
@@ -577,7 +580,8 @@ def main():
         for mname, nq in (("ibz", args.ibz_nq or (16 if big else None)), ("full_bz", args.full_nq or (2 if big else 8))):
             if mname == args.mode:
                 continue
-            w2 = Workload(args.workload, MODES[mname], B, pack, inp=wl.inp, nq_subset=nq, torch=torch, dev=dev, device_index=local)
+            w2 = Workload(args.workload, MODES[mname], B, pack, inp=wl.inp, nq_subset=nq, torch=torch, dev=dev, device_index=local,
+                          dv=getattr(wl, "dv", None))
             w2.lib.set_option("engine", args.engine)
             tt, k2, _, _ = run_steps(w2, torch, dev, 1, 1, timing=(mname == "ibz"))
             scale = w2.cfg.nk / w2.nq

@@ -245,21 +245,21 @@ __global__ void probe_mixed_kernel(long long iters, double* sink) {
 
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream) {
   if (ntarget <= 0) return cudaSuccess;
-  if (p.n <= 512) {
-    const int smem = UNF_NS * p.n * (int)sizeof(double2);          // 154 KB at naux = 300
+  constexpr int kMaxDyn = 227 * 1024 - 4096;                         // opt-in limit minus the kernel's static shared memory
+  const int smem = UNF_NS * p.n * (int)sizeof(double2);              // 154 KB at naux = 300
+  if (p.n <= 512 && smem <= kMaxDyn) {
     static bool attr_set[64] = {false};
     int dev = 0;
-    cudaGetDevice(&dev);
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-      cudaError_t e = cudaFuncSetAttribute(unfold_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, UNF_NS * 512 * (int)sizeof(double2) > 227 * 1024 ? 227 * 1024 : UNF_NS * 512 * (int)sizeof(double2));
+      e = cudaFuncSetAttribute(unfold_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDyn);
       if (e != cudaSuccess) return e;
       attr_set[dev] = true;
     }
-    if (smem <= 227 * 1024) {
-      dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n + UNF_RB - 1) / UNF_RB));
-      unfold_tiled_kernel<<<grid, 256, smem, stream>>>(p);
-      return cudaGetLastError();
-    }
+    dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n + UNF_RB - 1) / UNF_RB));
+    unfold_tiled_kernel<<<grid, 256, smem, stream>>>(p);
+    return cudaGetLastError();
   }
   dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n * p.n + 255) / 256));
   unfold_sparse_kernel<<<grid, 256, 0, stream>>>(p);
