@@ -46,6 +46,7 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--mode", default="ibz_block", choices=list(MODES))
     ap.add_argument("--no-modes", action="store_true", help="skip the FULL_BZ / IBZ comparison legs")
+    ap.add_argument("--no-p0", action="store_true", help="skip the bare-bubble (Eq. 20) leg")
     ap.add_argument("--no-cfg4", action="store_true", help="default workload only: skip the cfg4 sub-record (1 warm-up + 1 step, ~3 min)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
@@ -389,6 +390,70 @@ def fold_and_compare(wl, sigma_flat, ref, ks, taus):
     return worst
 
 
+def p0_leg(inp, B, pack, torch, dev, local, engine, dv, steps=2, warmup=1, with_oracle=True):
+    """N1: one bare-bubble evaluation P0^q(tau) (Eq. 20, Algorithm 3) for the wedge q of the same crystal, dense IBZ mode,
+    V^{k,k+q} for all Nk x nik pairs synthesised on the device (input generation) and resident; checked against
+    oracle/p0_oracle.py at one (q, tau) pair of outputs."""
+    lib = B.Gwsig(device=local)
+    cfg = pack.configure_from_crystal(lib, inp.cr, B.IBZ)
+    lib.set_option("engine", engine)
+    nk, nq = cfg.nk, len(cfg.out_list)
+    zero_w = np.zeros((1, 1, 1), complex)
+    G = np.ascontiguousarray(np.stack([inp.G_k(int(k)) for k in cfg.ir_list]).ravel(), np.complex128)
+    km = inp.kmesh
+    ks = [k for k in range(nk) for _ in range(nq)]
+    kqs = [int(km.index(km.n[k] + km.n[int(q)])) for k in range(nk) for q in cfg.out_list]
+    if dv is None:
+        dv = DeviceV(inp, torch, dev)
+    V = torch.empty((len(ks), dv.nel), dtype=torch.complex128, device=dev)
+    for s0 in range(0, len(ks), 256):
+        V[s0:s0 + 256] = dv.dense(ks[s0:s0 + 256], kqs[s0:s0 + 256])           # V^{k,k+q}: first momentum k, second k+q
+    dG = torch.from_numpy(G).to(dev)
+    dP = torch.zeros(nq * cfg.ntau * cfg.naux ** 2, dtype=torch.complex128, device=dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    lib.set_option("timing", 1)
+    for _ in range(warmup):
+        lib.p0_eval(dG, V, dP, stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        lib.p0_eval(dG, V, dP, stream)
+    e1.record()
+    e1.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    kinds = lib.kernel_times()
+    A_, B_ = float(cfg.naux) * cfg.nao ** 3, float(cfg.naux) ** 2 * cfg.nao ** 2
+    flops = 8.0 * nk * nq * cfg.ntau * (2 * A_ + B_)
+    rec = {"what": "bare bubble P0^q(tau), Eq. 20 / Algorithm 3, q in the wedge, dense blocks", "ms": ms, "pairs": nk * nq,
+           "gflop_algorithmic": flops / 1e9, "tflops": flops / (ms * 1e-3) / 1e12, "frac_fp64_tensor_peak": flops / (ms * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
+           "kernels_ms": {k: round(v[0], 2) for k, v in kinds.items() if v[1]}, "gpu_launches": int(lib.last_launch_count())}
+    if with_oracle:
+        from oracle.p0_oracle import p0_ref
+        iq, taus = nq - 1, [0, cfg.ntau // 2]
+        q = int(cfg.out_list[iq])
+        kq_of = lambda k: int(km.index(km.n[k] + km.n[q]))
+        Va = inp.V_pairs(list(range(nk)), [kq_of(k) for k in range(nk)])          # V^{k,k+q}
+        Vb = inp.V_pairs([kq_of(k) for k in range(nk)], list(range(nk)))          # V^{k+q,k}: generated independently
+        Gc = {}
+
+        def G_of(k):
+            if k not in Gc:
+                Gc[k] = inp.G_k(k)
+            return Gc[k]
+        t0 = time.perf_counter()
+        calls = {"n": 0}
+
+        def V_pair(a, b):            # p0_ref asks for V^{k,k+q} (first momentum k = a) first, then V^{k+q,k} (second momentum k = b)
+            calls["n"] += 1
+            return Va[a] if calls["n"] % 2 == 1 else Vb[b]
+        ref = p0_ref(nk, lambda k, q_: kq_of(k), G_of, V_pair, [q], taus)[0]
+        got = dP.cpu().numpy().reshape(nq, cfg.ntau, cfg.naux, cfg.naux)[iq][taus]
+        rec["parity_sample_max_rel_err"] = float(max(np.linalg.norm(got[i] - ref[i]) / np.linalg.norm(ref[i]) for i in range(len(taus))))
+        rec["parity_sample"] = f"q={q}, tau idx={taus}, oracle {time.perf_counter() - t0:.1f} s"
+    return rec
+
+
 def sample_points(cfg_ir_list, ntau, nk_sample, ntau_sample):
     ks = [int(cfg_ir_list[0]), int(cfg_ir_list[-1])][:nk_sample] if len(cfg_ir_list) > 1 else [int(cfg_ir_list[0])]
     taus = sorted(set(np.linspace(0, ntau - 1, ntau_sample).round().astype(int).tolist()))
@@ -607,6 +672,12 @@ def main():
             for m in modes.values():
                 m["speedup_vs_full_bz"] = base / m["ms"]
         line["modes"] = modes
+
+    # ---- N1: the bare bubble on the same crystal -------------------------------------------------------------------------------
+    if args.workload in ("cfg2", "cfg3") and not args.no_p0 and world == 1:
+        wl.V = None
+        torch.cuda.empty_cache()
+        line["p0"] = p0_leg(wl.inp, B, pack, torch, dev, local, args.engine, getattr(wl, "dv", None), with_oracle=not args.no_cpu_baseline)
 
     # ---- the other target config of the north star (configs 3-4): one step of cfg4 in the same job ------------------------------
     if args.workload == "cfg3" and not args.no_cfg4 and world == 1:

@@ -105,6 +105,10 @@ class RandomC1Inputs:
         """V^{k2,k1}_{Q,bj} for every k2 in k2s  [len, naux, nao, nao]"""
         return np.stack([self._V[k2, k1] for k2 in k2s])
 
+    def V_pairs(self, k1s, k2s) -> np.ndarray:
+        """V^{k1,k2}_{Q,ij} for a list of pairs  [len, naux, nao, nao]"""
+        return np.stack([self._V[a, b] for a, b in zip(k1s, k2s)])
+
     def V1_rows(self, k1: int, k2s) -> np.ndarray:
         """V^{k1,k2}_{Q,ia} for every k2 in k2s  [len, naux, nao, nao]"""
         return np.stack([self._V[k1, k2] for k2 in k2s])
@@ -314,6 +318,17 @@ class SymmetricInputs:
         f1 = np.exp(-2j * np.pi * (self.kmesh.frac[k2s] @ self.vR1.T))   # [nk2, nR1]
         return (f1 @ T).reshape(len(k2s), self.naux, self.nao, self.nao)
 
+
+    def V_pairs(self, k1s, k2s) -> np.ndarray:
+        """V^{k1,k2}_{Q,ij} for a LIST of pairs (k1s[n], k2s[n])  [len, naux, nao, nao]: the Bloch sum of V_pair with the two
+        phase vectors multiplied out per pair, as two real products against the real-space table."""
+        k1s, k2s = np.asarray(list(k1s)), np.asarray(list(k2s))
+        f1 = np.exp(-2j * np.pi * (self.kmesh.frac[k1s] @ self.vR1.T))         # [n, nR1]
+        f2 = np.exp(+2j * np.pi * (self.kmesh.frac[k2s] @ self.vR2.T))         # [n, nR2]
+        F = (f1[:, :, None] * f2[:, None, :]).reshape(len(k1s), -1)
+        Vd = self.Vd.reshape(F.shape[1], -1)
+        out = (F.real @ Vd) + 1j * (F.imag @ Vd)
+        return out.reshape(len(k1s), self.naux, self.nao, self.nao)
 
     def V1_rows(self, k1: int, k2s) -> np.ndarray:
         """V^{k1,k2}_{Q,ia} for every k2 in k2s  [len, naux, nao, nao]  (same Bloch sum as V_pair, batched over k2)."""
