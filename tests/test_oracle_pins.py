@@ -322,3 +322,43 @@ def test_p0_gauge_and_hermiticity():
     P0s = p0_ref(inp.nk, add, lambda k: G[k], Vaux, [q])[0]
     want = np.einsum("PQ,tQR,SR->tPS", S, P0[q], S.conj())
     assert np.abs(P0s - want).max() < 1e-13 * np.abs(P0).max()
+
+
+# ---- Eq. 27, block-basis transform of V ---------------------------------------------------
+def test_block_transform_brute_inverse_norm():
+    from oracle.block_oracle import block_transform_brute, block_transform_ref
+    rng = np.random.default_rng(9)
+    u = lambda n: np.linalg.qr(rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n)))[0]
+    V = rng.standard_normal((4, 3, 3)) + 1j * rng.standard_normal((4, 3, 3))
+    Ux, U2, U1 = u(4), u(3), u(3)
+    a, b = block_transform_brute(V, Ux, U2, U1), block_transform_ref(V, Ux, U2, U1)
+    assert np.abs(a - b).max() < 1e-14
+    assert abs(np.linalg.norm(b) - np.linalg.norm(V)) < 1e-13                         # unitary change of basis
+    back = np.einsum("QP,ba,Pai,ji->Qbj", Ux, U2, b, U1.conj())                       # the inverse of Eq. 27 written out
+    assert np.abs(back - V).max() < 1e-13
+
+
+def test_block_transform_makes_sigma_covariant():
+    """Sigma from block-basis inputs (Eq. 26 for G and W, Eq. 27 for BOTH V tensors) = U^dagger Sigma U: fixes which index of V
+    carries which conjugation, against the independently pinned sigma_ref."""
+    from oracle.block_oracle import block_transform_ref
+    from oracle.sigma_oracle import sigma_ref
+    inp = make_inputs("cfg1", mesh=(2, 2, 1), nao=3, naux=4, ntau=2, beta=3.0, nocc=1, seed=6)
+    G, W = inp.G_full(), inp.W_full()
+    rng = np.random.default_rng(5)
+    u = lambda n: np.linalg.qr(rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n)))[0]
+    U = [u(3) for _ in range(inp.nk)]
+    Ux = [u(4) for _ in range(inp.nk)]
+    sub = lambda a, b: int(inp.kmesh.sub(a, b))
+    ks = list(range(inp.nk))
+    S = sigma_ref(inp.nk, sub, lambda k: G[k], lambda q: W[q], inp.V_pair, ks)
+    # V_pair(k1, k2) = V^{k1,k2}: first momentum k1, second k2, auxiliary momentum q = k2 - k1 -> Eq. 27 with (k2 -> k1, k1 -> k2)
+    Vb = lambda k1, k2: block_transform_ref(inp.V_pair(k1, k2), Ux[sub(k2, k1)], U[k1], U[k2])
+    # W^q_{QQ'}: Q contracts with the V of auxiliary momentum -q, Q' with the one of +q (reading A6); both carry conj(U_aux) from
+    # Eq. 27, so the matching two-index object is W_blk[P,P'] = sum_{QQ'} Uaux^{-q}_{Q,P} W_{QQ'} Uaux^{q}_{Q',P'}
+    def Wb(q):
+        return np.einsum("QP,tQR,RS->tPS", Ux[sub(0, q)], W[q], Ux[q])
+    Sb = sigma_ref(inp.nk, sub, lambda k: U[k].conj().T @ G[k] @ U[k], Wb, Vb, ks)
+    for k in ks:
+        want = U[k].conj().T @ S[k] @ U[k]
+        assert np.abs(Sb[k] - want).max() < 1e-12 * np.abs(S).max()
