@@ -63,7 +63,8 @@ enum {
   GWSIG_KIND_STAGE2 = 3, /* Y = W X          */
   GWSIG_KIND_STAGE3 = 4, /* Sigma += Y V     */
   GWSIG_KIND_EPILOGUE = 5,
-  GWSIG_NKINDS = 6
+  GWSIG_KIND_VTRANSFORM = 6, /* Eq. 27 block transform of V (gwsig_block_transform_v) */
+  GWSIG_NKINDS = 7
 };
 
 /* ---- life cycle ------------------------------------------------------------------------ */
@@ -175,6 +176,15 @@ int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, co
 int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream);
 int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream);
 
+/* ---- N4: block-basis transform of V on the device ----------------------------------------
+ * V2blk_{P,a,i} = sum_{Q,b,j} conj(Uaux^q_{Q,P}) conj(U^{k2}_{b,a}) V2_{Q,b,j} U^{k1}_{j,i}     (Eq. 27; V2 = V^{k2,k1},
+ * q = k1 - k2) for pairs p0 .. p0+np-1: dV_dense (dev) holds the orbital-basis tensors [naux][nao][nao] back to back in pair
+ * order, dV_packed (dev) receives the allowed blocks in the packed layout sigma_push_pairs expects (first element = first
+ * element of pair p0).  Needs GWSIG_IBZ_BLOCK, set_blocks WITH U_ao / U_aux, set_triples.  Three launches of the grouped engine
+ * per sub-batch of pairs (auxiliary index, first orbital index, second orbital index + packing); the paper does this step on
+ * the CPU before the calculation.  Synchronises the stream.                                              */
+int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, void* dV_packed, void* stream);
+
 /* ---- N1: bare bubble ---------------------------------------------------------------
  * P0^q_{QQ'}(tau) = -(1/Nk) sum_k sum_{abcd} V^{k,k+q}_{Q,da} G^k_{cd}(-tau) G^{k+q}_{ab}(tau) V^{k+q,k}_{Q',bc}   (Eq. 20,
  * PAPER.md:179-184; one spin channel) in the order of Algorithm 3: X1 = V G^k(-tau), X2 = V G^{k+q}(tau),
@@ -216,7 +226,7 @@ int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
 int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
- * stage: 31, 32, 33 = the three stages of the bare bubble (p0 / np then count P0 pairs); 11, 12 / 21, 22 = the two launches of
+ * stage: 41, 42, 43 = the three steps of the Eq. 27 transform (gwsig_block_transform_v); 31, 32, 33 = the three stages of the bare bubble (p0 / np then count P0 pairs); 11, 12 / 21, 22 = the two launches of
  * the Eq. 28 block unfold of G / W (p0 = first mesh point, np = number of points); 1 = X = V G lowered transposed, X^T = G^T conj(V2) (A = G, B = V2, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
  * B = W, C = Y), 3 = Sigma += Y V (A = Y, B = V2, C = Sigma accumulator; the segment list of an
  * output block may be cut into several problems that add into the same C).

@@ -75,6 +75,7 @@ struct gwsig_ctx {
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
   DevBuf oblk_ao, oblk_aux, unf_tmp, partial;
+  DevBuf u_ao_dev, u_aux_dev;                    // N4: the adapted bases on the device (set_blocks with U)
   DevBuf grev, p0acc, p0desc;                    // N1 (Eq. 20): G(beta - tau) on the full zone, the P0 accumulator, its epilogue descriptors
   bool in_p0 = false;
   double2* dP0 = nullptr;
@@ -205,6 +206,11 @@ int prepare_tables(gwsig_ctx* ctx) {
     if ((rc = upload(ctx, ctx->colphase_aux, ph))) return rc;
     if ((rc = upload(ctx, ctx->tgt_src, src))) return rc;
     if ((rc = upload(ctx, ctx->tgt_op, op))) return rc;
+  }
+  if (P.mode == GWSIG_IBZ_BLOCK && P.have_U) {
+    int rc;
+    if ((rc = upload(ctx, ctx->u_ao_dev, P.U_ao))) return rc;
+    if ((rc = upload(ctx, ctx->u_aux_dev, P.U_aux))) return rc;
   }
   if (P.mode == GWSIG_IBZ_BLOCK && P.general_gauge) {
     int rc;
@@ -374,7 +380,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -543,7 +549,8 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
   const Plan& P = ctx->plan;
   if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
+  int rc = stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
+         : stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
          : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_counts: bad range / stage");
@@ -558,7 +565,8 @@ int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, vo
   const Plan& P = ctx->plan;
   if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
+  int rc = stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
+         : stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
          : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
   if (rc) return fail(ctx, rc, "plan_get: bad range / stage");
@@ -763,6 +771,58 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
   rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
   if (rc) { ctx->in_eval = false; ctx->exchange = false; return rc; }
   return gwsig_sigma_end(ctx);
+}
+
+/* ---- N4: Eq. 27 on the device --------------------------------------------------------------------------- */
+int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, void* dV_packed, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (P.mode != GWSIG_IBZ_BLOCK || !P.have_blocks || !P.have_triples)
+    return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: needs GWSIG_IBZ_BLOCK with set_blocks and set_triples");
+  if (!P.have_U) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: set_blocks must be given the adapted bases U_ao, U_aux");
+  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "block_transform_v: an evaluation is open");
+  if (np < 1 || p0 < 0 || p0 + np > P.npairs) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: bad pair range");
+  if (!dV_dense || !dV_packed) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: NULL device pointer");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)stream;
+  if ((rc = prepare_tables(ctx))) return rc;
+  CU(ctx->counters.ensure(gwsig_ctx::kCounterSlots * sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
+  ctx->counter_slot = 0;
+  const long long xs = (long long)P.naux * P.nao * P.nao;
+  size_t free_b = 0, total_b = 0;
+  CU(cudaMemGetInfo(&free_b, &total_b));
+  const double avail = 0.4 * ((double)free_b + (double)ctx->xbuf.bytes + (double)ctx->ybuf.bytes);
+  const double budget = std::min((double)ctx->scratch_mib * 1048576.0, std::max(avail, 64.0 * 1048576.0)) / (2.0 * sizeof(double2));
+  const long long ns_max = std::max<long long>(1, (long long)(budget / (double)xs));
+  for (long long s0 = p0; s0 < p0 + np; s0 += ns_max) {
+    const long long ns = std::min<long long>(ns_max, p0 + np - s0);
+    CU(ctx->xbuf.ensure((size_t)xs * ns * sizeof(double2)));
+    CU(ctx->ybuf.ensure((size_t)xs * ns * sizeof(double2)));
+    const double2* Vsub = (const double2*)dV_dense + (s0 - p0) * xs;
+    double2* Out = (double2*)dV_packed + (P.v_off[s0] - P.v_off[p0]);
+    for (int step = 1; step <= 3; ++step) {
+      StagePlan sp;
+      rc = P.build_vtransform(s0, ns, step, sp);
+      if (rc) return fail(ctx, rc, "internal: build_vtransform failed");
+      DevStage d;
+      d.nprob = (int)sp.prob.size(); d.ntiles = sp.ntiles;
+      if ((rc = upload(ctx, d.prob, sp.prob))) return rc;
+      if ((rc = upload(ctx, d.seg, sp.seg))) return rc;
+      if ((rc = upload(ctx, d.bucket, sp.bucket))) return rc;
+      const double2* A = step == 1 ? Vsub : step == 2 ? (const double2*)ctx->xbuf.p : (const double2*)ctx->ybuf.p;
+      const double2* Bm = (const double2*)(step == 1 ? ctx->u_aux_dev.p : ctx->u_ao_dev.p);
+      double2* C = step == 1 ? (double2*)ctx->xbuf.p : step == 2 ? (double2*)ctx->ybuf.p : Out;
+      rc = run_stage(ctx, GWSIG_KIND_VTRANSFORM, d, A, Bm, C, 0);
+      cudaError_t e = cudaStreamSynchronize(ctx->stream);      // the descriptor tables are freed below
+      d.prob.release(); d.seg.release(); d.bucket.release();
+      if (rc) return rc;
+      if (e != cudaSuccess) return cuda_fail(ctx, e, "block_transform_v");
+    }
+  }
+  return GWSIG_OK;
 }
 
 /* ---- N1: bare bubble P0^q(tau) (Eq. 20, Algorithm 3), dense modes ---------------------------- */

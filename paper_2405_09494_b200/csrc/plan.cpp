@@ -168,7 +168,7 @@ int Plan::set_symmetry(int nops_, const int* rot_, const double* trans_, const d
   // trivial (one-block) maps; set_blocks overrides them in IBZ_BLOCK mode
   ao_off.assign(nk, std::vector<int>{0, nao});
   aux_off.assign(nk, std::vector<int>{0, naux});
-  U_ao.clear(); U_aux.clear(); general_gauge = false;
+  U_ao.clear(); U_aux.clear(); general_gauge = false; have_U = false;
   have_sym = true;
   have_blocks = have_triples = false;
   triple_ptr.clear(); triples.clear();
@@ -225,7 +225,23 @@ int Plan::set_blocks(const int* nblk_ao, const int* ao_block_off, const int* nbl
     U_aux.assign(ux, ux + (size_t)nk * naux * naux);
     if ((rc = compute_oblock(false))) return rc;
     if ((rc = compute_oblock(true))) return rc;
+    // U given in the gauge U^{k'} = O U^{k_I}: every O_block is the identity and nothing has to be unfolded
+    auto is_identity = [&](const std::vector<cplx>& ob, const std::vector<long long>& oo, const std::vector<std::vector<int>>& offs) {
+      for (int k = 0; k < nk; ++k) {
+        long long o = oo[k];
+        for (size_t b = 0; b + 1 < offs[k].size(); ++b) {
+          const int nb = offs[k][b + 1] - offs[k][b];
+          for (int r = 0; r < nb; ++r)
+            for (int c = 0; c < nb; ++c)
+              if (std::abs(ob[(size_t)o + (size_t)r * nb + c] - cplx(r == c ? 1.0 : 0.0, 0.0)) > 1e-10) return false;
+          o += (long long)nb * nb;
+        }
+      }
+      return true;
+    };
+    if (is_identity(oblk_ao, oblk_ao_off, ao_off) && is_identity(oblk_aux, oblk_aux_off, aux_off)) general_gauge = false;
   } else { U_ao.clear(); U_aux.clear(); oblk_ao.clear(); oblk_aux.clear(); }
+  have_U = U_ao_ != nullptr;
   have_blocks = true;
   have_triples = false;
   triple_ptr.clear(); triples.clear();
@@ -700,6 +716,89 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
       bo += (long long)nb * nb;
     }
     uoff += ts * ntau;
+  }
+  long long tb = 0;
+  for (auto& P : out.prob) {
+    P.tiles_m = zg_tiles_m(P.M, tile_m[0]);
+    P.tiles_n = zg_tiles_n(P.N);
+    P.tile_begin = tb;
+    tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
+  }
+  out.ntiles = tb;
+  out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
+  size_t pi = 0;
+  for (size_t bkt = 0; bkt < out.bucket.size(); ++bkt) {
+    const long long t = (long long)bkt << ZG_BUCKET_SHIFT;
+    while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
+    out.bucket[bkt] = (int)pi;
+  }
+  return GWSIG_OK;
+}
+
+int Plan::build_vtransform(long long p0, long long np, int step, StagePlan& out) const {
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
+  if (mode != GWSIG_IBZ_BLOCK || !have_U || !have_triples) return GWSIG_ERR_ARG;
+  if (p0 < 0 || np < 1 || p0 + np > npairs || step < 1 || step > 3) return GWSIG_ERR_ARG;
+  const long long n2 = (long long)nao * nao, xs = (long long)naux * n2;
+  for (long long l = 0; l < np; ++l) {
+    const long long p = p0 + l;
+    int k1, k2, q, i1;
+    pair(p, k1, k2, q, i1);
+    if (step < 3) {
+      gwsig_seg S; std::memset(&S, 0, sizeof(S));
+      gwsig_problem P; std::memset(&P, 0, sizeof(P));
+      S.a_off = l * xs; P.c_off = l * xs;
+      if (step == 1) {        // T1^T[(b,j), P] = sum_Q V2^T[(b,j), Q] conj(Uaux^q)[Q, P]
+        S.am = lvl1(1); S.ak = lvl1(n2);
+        S.b_off = (long long)q * naux * naux; S.bk = lvl1(naux); S.bn = lvl1(1);
+        S.K = naux;
+        P.M = (int)n2; P.N = naux;
+        P.cm = lvl1(1); P.cn = lvl1(n2);
+      } else {                // T2[(P,j), a] = sum_b T1[P][b][j] conj(U^{k2})[b, a]
+        S.am = lvl2(nao, n2, 1); S.ak = lvl1(nao);
+        S.b_off = (long long)k2 * n2; S.bk = lvl1(nao); S.bn = lvl1(1);
+        S.K = nao;
+        P.M = naux * nao; P.N = nao;
+        P.cm = lvl2(nao, n2, 1); P.cn = lvl1(nao);
+      }
+      P.flags = GWSIG_FLAG_CONJ_B;
+      P.nbatch = 1;
+      P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+      out.seg.push_back(S); out.prob.push_back(P);
+    } else {
+      const std::vector<int>&oq = aux_off[q], &o2 = ao_off[k2], &o1 = ao_off[k1];
+      const int nb = (int)oq.size() - 1;
+      std::vector<long long> Np(nb, 0), c0s;
+      const int ntr = pair_ntriples(p);
+      c0s.resize(ntr);
+      for (int t = 0; t < ntr; ++t) {
+        int bp, ba, bi;
+        pair_triple(p, t, bp, ba, bi);
+        c0s[t] = Np[bp];
+        Np[bp] += (long long)(o2[ba + 1] - o2[ba]) * (o1[bi + 1] - o1[bi]);
+      }
+      std::vector<long long> poff(nb + 1, 0);
+      for (int b = 0; b < nb; ++b) poff[b + 1] = poff[b] + (long long)(oq[b + 1] - oq[b]) * Np[b];
+      for (int t = 0; t < ntr; ++t) {
+        int bp, ba, bi;
+        pair_triple(p, t, bp, ba, bi);
+        const int n_p = oq[bp + 1] - oq[bp], na = o2[ba + 1] - o2[ba], ni = o1[bi + 1] - o1[bi];
+        gwsig_seg S; std::memset(&S, 0, sizeof(S));
+        gwsig_problem P; std::memset(&P, 0, sizeof(P));
+        // packed(P,a,i) = sum_j T2[oq+P][o2+a][j] U^{k1}[j][o1+i]
+        S.a_off = l * xs + (long long)oq[bp] * n2 + (long long)o2[ba] * nao;
+        S.am = lvl2(na, n2, nao); S.ak = lvl1(1);
+        S.b_off = (long long)k1 * n2 + o1[bi]; S.bk = lvl1(nao); S.bn = lvl1(1);
+        S.K = nao;
+        P.M = n_p * na; P.N = ni;
+        P.c_off = (v_off[p] - v_off[p0]) + poff[bp] + c0s[t];
+        P.cm = lvl2(na, Np[bp], ni); P.cn = lvl1(1);
+        P.flags = 0;
+        P.nbatch = 1;
+        P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+        out.seg.push_back(S); out.prob.push_back(P);
+      }
+    }
   }
   long long tb = 0;
   for (auto& P : out.prob) {

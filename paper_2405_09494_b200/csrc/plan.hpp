@@ -60,7 +60,8 @@ struct Plan {
   // ---- blocks (IBZ_BLOCK) -------------------------------------------------------------------
   std::vector<std::vector<int>> ao_off, aux_off;     // per k: nblk+1 offsets (trivial {0,n} in dense modes)
   std::vector<cplx> U_ao, U_aux;                     // optional explicit gauge (set_blocks with U)
-  bool general_gauge = false;
+  bool general_gauge = false;                        // O_block != 1 somewhere: packed G / W must be unfolded (Eq. 28)
+  bool have_U = false;                               // set_blocks was given U (needed by the Eq. 27 transform, N4)
   // O_block = U^{k'}^dagger O^{k_I}(alpha^) U^{k_I} (Eq. 28) for op_of[k'], packed diagonal blocks per mesh
   // point (block b of point k at oblk_*_off[k] + blk_off(b), row-major); only in the explicit gauge
   std::vector<cplx> oblk_ao, oblk_aux;
@@ -138,6 +139,11 @@ struct Plan {
   // stage 1: X1[(c,a)][Q] = sum_d Grev^k[c,d] T[Q,d,a]   (Grev(tau_n) = G(beta - tau_n): G(-tau) = -Grev, sign in the epilogue)
   // stage 2: X2[(c,a)][Q'] = sum_b G^{kq}[a,b] conj(T[Q',c,b])
   // stage 3: P0acc[iq][tau][Q][Q'] += sum over the pairs of the range with that q, sum_{(c,a)} X1[(c,a)][Q] X2[(c,a)][Q']
+  // ---- N4: Eq. 27 on the device: dense orbital-basis V2 of pairs p0.. -> packed block-basis V2 (allowed triples)
+  //   step 1  T1[P][(b,j)] = sum_Q conj(Uaux^q[Q,P]) V2[Q][(b,j)]      step 2  T2[P][a][j] = sum_b conj(U^{k2}[b,a]) T1[P][b][j]
+  //   step 3  packed(P,a,i) = sum_j T2[P][a][j] U^{k1}[j,i]   for the allowed triples only, written in the packed layout
+  // A: dense V2 / T1 / T2 (pair l at l * naux * nao^2), B: the U_aux table (step 1) or the U_ao table (steps 2, 3), [Nk][n][n]
+  int build_vtransform(long long p0, long long np, int step, StagePlan& out) const;
   int build_p0_stage(long long p0, long long np, int nt, int stage, StagePlan& out, int num_sms = 148) const;
 };
 

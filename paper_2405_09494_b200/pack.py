@@ -15,7 +15,7 @@ class Configured:
     """a Gwsig context with lattice / symmetry (/ blocks) set, plus the host pre-step objects."""
 
     def __init__(self, lib: Gwsig, mode: int, a, mesh, nao, naux, ntau, beta, pos, ao_atom, aux_atom,
-                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7, out_points=None, scramble_gauge=None):
+                 W=None, w=None, shift=None, P_ao=None, P_aux=None, seed: int = 7, out_points=None, scramble_gauge=None, pass_U=False):
         self.lib, self.mode = lib, mode
         self.general_gauge = scramble_gauge is not None and mode == IBZ_BLOCK
         self.nao, self.naux, self.ntau = nao, naux, ntau
@@ -40,7 +40,9 @@ class Configured:
         self.out_list = (np.arange(self.nk) if mode == FULL_BZ else self.ir_list) if out_points is None else np.asarray(out_points)
         if mode == IBZ_BLOCK:
             self.ao, self.aux = self.setup.adapt("ao"), self.setup.adapt("aux")
-            if scramble_gauge is None:
+            if scramble_gauge is None and pass_U:
+                lib.set_blocks(self.ao.off, self.aux.off, self.ao.U, self.aux.U)     # gauge S5 with U handed over (for Eq. 27 on the device)
+            elif scramble_gauge is None:
                 lib.set_blocks(self.ao.off, self.aux.off)                 # gauge S5: O_block = 1, no U needed
             else:                                                         # general gauge: the library forms O_block (Eq. 28)
                 self.ao = self.setup.scramble(self.ao, scramble_gauge)
@@ -107,9 +109,9 @@ class Configured:
         return out
 
 
-def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7, out_points=None, scramble_gauge=None) -> Configured:
+def configure_from_crystal(lib: Gwsig, cr, mode: int, seed: int = 7, out_points=None, scramble_gauge=None, pass_U=False) -> Configured:
     """convenience for the synthetic crystals of gwsig_synth (any object with the same fields)."""
     sg = cr.sg
     return Configured(lib, mode, cr.a, cr.mesh, cr.nao, cr.naux, cr.ntau, cr.beta, cr.pos, cr.ao_atom, cr.aux_atom,
                       W=sg.W, w=sg.w, shift=sg.shift, P_ao=cr.P_ao, P_aux=cr.P_aux, seed=seed, out_points=out_points,
-                      scramble_gauge=scramble_gauge)
+                      scramble_gauge=scramble_gauge, pass_U=pass_U)

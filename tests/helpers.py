@@ -295,3 +295,36 @@ def run_p0_plan_numpy(cfg, inp, G_flat, V_flat, push_pairs=None, nt=None):
             run_stage_numpy(pr, sg, X1, X2, acc, t0)
         p0 += npp
     return (acc / nk).reshape(nq, ntau, naux, naux)
+
+
+# ---- N4: Eq. 27 on the device ----------------------------------------------------------------------------------
+def oracle_packed_V(cfg, inp, pairs):
+    """oracle/block_oracle.block_transform_ref of V2 = V^{k2,k1} for the given pairs, packed by the layout include/gwsig.h
+    documents (aux block p major, [n_p][N_p], segments [a][i] in triple order) -- written out here, not taken from the package."""
+    from oracle.block_oracle import block_transform_ref
+    out = []
+    for p in pairs:
+        k1, k2, q, _, _ = cfg.lib.pair_info(p, with_layout=False)
+        T = block_transform_ref(inp.V2_rows(k1, [k2])[0], cfg.aux.U[q], cfg.ao.U[k2], cfg.ao.U[k1])
+        oq, o2, o1 = cfg.aux.off[q], cfg.ao.off[k2], cfg.ao.off[k1]
+        trip = cfg.triples[p]
+        for bp in range(len(oq) - 1):
+            segs = [T[oq[bp]:oq[bp + 1], o2[a]:o2[a + 1], o1[i]:o1[i + 1]].reshape(oq[bp + 1] - oq[bp], -1) for (pp, a, i) in trip if pp == bp]
+            if segs:
+                out.append(np.concatenate(segs, axis=1).ravel())
+    return np.concatenate(out)
+
+
+def run_vtransform_numpy(cfg, inp, p0, npairs):
+    """the three launches of gwsig_block_transform_v (plan stages 41, 42, 43) with the numpy interpreter."""
+    lib = cfg.lib
+    xs = cfg.naux * cfg.nao ** 2
+    info = [lib.pair_info(p) for p in range(p0, p0 + npairs)]
+    V = np.concatenate([inp.V2_rows(i[0], [i[1]])[0].ravel() for i in info])
+    Uaux, Uao = np.ascontiguousarray(cfg.aux.U).ravel(), np.ascontiguousarray(cfg.ao.U).ravel()
+    T1, T2 = np.zeros(npairs * xs, complex), np.zeros(npairs * xs, complex)
+    out = np.zeros(sum(i[4] for i in info), complex)
+    for step, (A, Bm, C) in enumerate(((V, Uaux, T1), (T1, Uao, T2), (T2, Uao, out)), 1):
+        pr, sg, _ = lib.plan_get(p0, npairs, 1, 40 + step)
+        run_stage_numpy(pr, sg, A, Bm, C, 0)
+    return out

@@ -4,7 +4,7 @@ FP64, after folding the result back to the orbital basis."""
 import numpy as np
 import pytest
 
-from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_p0, oracle_sigma, pack_V_p0, rel_err
+from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_p0, oracle_packed_V, oracle_sigma, pack_V_p0, rel_err
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -322,6 +322,36 @@ def test_p0_eq20(name, mode):
         got = dP.cpu().numpy().reshape(shape)
         worst = max(rel_err(got[i, t], ref[i, t]) for i in range(nq) for t in range(inp.ntau))
         assert worst <= TOL, (variant, worst)
+
+
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite", "cfg2"])
+def test_block_transform_v_eq27(name):
+    """N4: gwsig_block_transform_v (Eq. 27: dense orbital-basis V2 -> packed block-basis V2 on the device) against
+    oracle/block_oracle.py, and the Sigma evaluated from that device-packed V against the Sigma oracle."""
+    B = _B()
+    torch = _torch()
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    inp = get_inputs(name)
+    lib = B.Gwsig(device=0)
+    cfg = configure_from_crystal(lib, inp.cr, 2, pass_U=True)
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    Vnp = cfg.pack_V(inp.V2_rows)                           # numpy pre-step: finds the triples (set_triples); its V is NOT used below
+    dense = np.concatenate([inp.V2_rows(lib.pair_info(p)[0], [lib.pair_info(p)[1]])[0].ravel() for p in range(cfg.npairs)])
+    dD = torch.from_numpy(dense).cuda()
+    dP = torch.full((Vnp.size,), float("nan"), dtype=torch.complex128, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    half = cfg.npairs // 2
+    lib.block_transform_v(0, half, dD, dP, stream)                                         # two calls: offsets of a later range
+    xs = inp.naux * inp.nao ** 2
+    lib.block_transform_v(half, cfg.npairs - half, dD[half * xs:], dP[lib.pair_info(half)[3]:], stream)
+    torch.cuda.synchronize()
+    got = dP.cpu().numpy()
+    sample = list(range(0, cfg.npairs, max(1, cfg.npairs // 25)))
+    voff = [lib.pair_info(p)[3] for p in range(cfg.npairs)] + [Vnp.size]
+    for p in sample:
+        ref = oracle_packed_V(cfg, inp, [p])
+        assert np.abs(got[voff[p]:voff[p + 1]] - ref).max() <= 1e-13 * np.abs(dense).max()
+    _check(cfg, inp, run_gpu(cfg, G, W, got), ks=None if inp.nk <= 64 else list(range(0, inp.nk, 7)))
 
 
 def test_output_point_subset_matches_full_run():

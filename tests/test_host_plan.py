@@ -230,3 +230,21 @@ def test_p0_plan_matches_oracle(name, mode):
     ref = oracle_p0(inp, cfg.out_list)
     scale = np.abs(ref).max()
     assert np.abs(got - ref).max() < 1e-12 * scale
+
+
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite"])
+def test_vtransform_plan_matches_oracle(name):
+    """N4 (Eq. 27): the three launches of gwsig_block_transform_v, run by the numpy interpreter, give the packed
+    block-basis V2 that oracle/block_oracle.py gives (packed by the documented layout); U handed over in the S5 gauge is
+    recognised (no unfold is planned: O_block = 1)."""
+    from tests.helpers import oracle_packed_V, run_vtransform_numpy
+    inp = make_inputs(name)
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ_BLOCK, pass_U=True)
+    cfg.pack_V(inp.V2_rows)                               # finds the allowed triples and calls set_triples
+    p0, n = 5, 11
+    got = run_vtransform_numpy(cfg, inp, p0, n)
+    ref = oracle_packed_V(cfg, inp, range(p0, p0 + n))
+    assert got.shape == ref.shape and np.abs(got - ref).max() < 1e-13 * np.abs(ref).max()
+    with pytest.raises(B.GwsigError):                      # S5 gauge recognised: the Eq. 28 unfold stages are not available
+        lib.plan_get(0, 4, inp.ntau, 11)
