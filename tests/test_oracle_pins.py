@@ -362,3 +362,34 @@ def test_block_transform_makes_sigma_covariant():
     for k in ks:
         want = U[k].conj().T @ S[k] @ U[k]
         assert np.abs(Sb[k] - want).max() < 1e-12 * np.abs(S).max()
+
+
+# ---- Eq. 19: P = [1 - P0]^{-1} P0 per (q, Omega) with caller-supplied tau <-> i Omega transforms ------
+def test_dyson_p_loops_scalar_series_resolvent():
+    from oracle.dyson_oracle import dyson_p_loops, dyson_p_ref
+    rng = np.random.default_rng(12)
+    nq, ntau, nw, n = 2, 5, 4, 3
+    P0 = 0.2 * (rng.standard_normal((nq, ntau, n, n)) + 1j * rng.standard_normal((nq, ntau, n, n)))
+    Tf = rng.standard_normal((nw, ntau)) + 1j * rng.standard_normal((nw, ntau))
+    Tb = rng.standard_normal((ntau, nw)) + 1j * rng.standard_normal((ntau, nw))
+    a, b = dyson_p_loops(P0, Tf, Tb), dyson_p_ref(P0, Tf, Tb)
+    assert np.abs(a - b).max() < 1e-12 * np.abs(b).max()
+    # scalar closed form, identity transforms: P = p0 / (1 - p0)
+    p0 = np.array([0.3 - 0.2j, -1.7 + 0.4j, 0.05j]).reshape(1, 3, 1, 1)
+    P = dyson_p_ref(p0, np.eye(3), np.eye(3))
+    assert np.abs(P - p0 / (1 - p0)).max() < 1e-15
+    # geometric series (small norm) and the resolvent identity, one frequency, identity transforms
+    A = 0.1 * (rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4)))
+    P = dyson_p_ref(A.reshape(1, 1, 4, 4), np.eye(1), np.eye(1))[0, 0]
+    series = sum(np.linalg.matrix_power(A, k) for k in range(1, 40))
+    assert np.abs(P - series).max() < 1e-14
+    assert np.abs(P - A - A @ P).max() < 1e-15 and np.abs(P - A - P @ A).max() < 1e-15
+    # the transforms act linearly on either side of the solve: diagonal (commuting) P0 goes through entry by entry
+    d = 0.3 * (rng.standard_normal((1, ntau, 2)) + 1j * rng.standard_normal((1, ntau, 2)))
+    P0d = np.zeros((1, ntau, 2, 2), complex)
+    P0d[..., 0, 0], P0d[..., 1, 1] = d[..., 0], d[..., 1]
+    Pd = dyson_p_ref(P0d, Tf, Tb)
+    for j in range(2):
+        w = Tf @ d[0, :, j]
+        assert np.abs(Pd[0, :, j, j] - Tb @ (w / (1 - w))).max() < 1e-13
+    assert np.abs(Pd[..., 0, 1]).max() == 0
