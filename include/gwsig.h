@@ -64,7 +64,9 @@ enum {
   GWSIG_KIND_STAGE3 = 4, /* Sigma += Y V     */
   GWSIG_KIND_EPILOGUE = 5,
   GWSIG_KIND_VTRANSFORM = 6, /* Eq. 27 block transform of V (gwsig_block_transform_v) */
-  GWSIG_NKINDS = 7
+  GWSIG_KIND_GRIDXFORM = 7,  /* tau <-> i Omega transforms of gwsig_dyson_p                  */
+  GWSIG_KIND_DYSON = 8,      /* batched [1 - P0]^{-1} P0 solve of gwsig_dyson_p             */
+  GWSIG_NKINDS = 9
 };
 
 /* ---- life cycle ------------------------------------------------------------------------ */
@@ -176,6 +178,18 @@ int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, co
 int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream);
 int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream);
 
+/* ---- N3: the auxiliary function P from the bare bubble ------------------------------------
+ * P^q(i Omega_n) = [1 - P0^q(i Omega_n)]^{-1} P0^q(i Omega_n)  (Eq. 19a),  P^q(tau) by the inverse transform
+ * (Eq. 19b), for every q of the output list (the paper does this step on the CPU with MPI).
+ * The tau <-> i Omega transforms are MATRICES supplied by the caller (the paper uses sparse intermediate-representation
+ * grids; on a plain grid Tb[t][n] = exp(-i Omega_n tau_t) / beta):
+ *   dP0 (dev) [nq][ntau][naux][naux]   dTf (dev) [nw][ntau]   dTb (dev) [ntau][nw]   dP (dev) [nq][ntau][naux][naux]
+ *   P0(i Omega_n) = sum_t Tf[n][t] P0(tau_t);   P(tau_t) = sum_n Tb[t][n] P(i Omega_n).
+ * Both transforms run on the grouped engine, the solve is a batched Gauss-Jordan elimination with partial pivoting (one CTA
+ * per (q, Omega) at a time).  Dense layouts only (GWSIG_FULL_BZ, GWSIG_IBZ).  Synchronises the stream; GWSIG_ERR_ARG if some
+ * 1 - P0(i Omega) is singular.                                                                                       */
+int gwsig_dyson_p(gwsig_ctx* ctx, const void* dP0, const void* dTf, const void* dTb, int nw, void* dP, void* stream);
+
 /* ---- N4: block-basis transform of V on the device ----------------------------------------
  * V2blk_{P,a,i} = sum_{Q,b,j} conj(Uaux^q_{Q,P}) conj(U^{k2}_{b,a}) V2_{Q,b,j} U^{k1}_{j,i}     (Eq. 27; V2 = V^{k2,k1},
  * q = k1 - k2) for pairs p0 .. p0+np-1: dV_dense (dev) holds the orbital-basis tensors [naux][nao][nao] back to back in pair
@@ -226,7 +240,7 @@ int gwsig_last_launch_count(gwsig_ctx* ctx, int64_t* launches);
 int gwsig_kernel_times(gwsig_ctx* ctx, double* ms, int64_t* launches);
 
 /* ---- plan introspection (host-only; used by the CPU tests of the host logic) -------------------
- * stage: 41, 42, 43 = the three steps of the Eq. 27 transform (gwsig_block_transform_v); 31, 32, 33 = the three stages of the bare bubble (p0 / np then count P0 pairs); 11, 12 / 21, 22 = the two launches of
+ * stage: 51 = a grid transform of gwsig_dyson_p (np = n_in, nt = n_out); 41, 42, 43 = the three steps of the Eq. 27 transform (gwsig_block_transform_v); 31, 32, 33 = the three stages of the bare bubble (p0 / np then count P0 pairs); 11, 12 / 21, 22 = the two launches of
  * the Eq. 28 block unfold of G / W (p0 = first mesh point, np = number of points); 1 = X = V G lowered transposed, X^T = G^T conj(V2) (A = G, B = V2, C = X), 2 = Y = W X lowered transposed, Y^T = X^T W (A = X,
  * B = W, C = Y), 3 = Sigma += Y V (A = Y, B = V2, C = Sigma accumulator; the segment list of an
  * output block may be cut into several problems that add into the same C).

@@ -36,7 +36,7 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
            "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host",
            "gwsig_set_output_points", "gwsig_exchange_begin", "gwsig_exchange_eval",
-           "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval", "gwsig_block_transform_v"]
+           "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval", "gwsig_block_transform_v", "gwsig_dyson_p"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -55,6 +55,7 @@ _sig = {
     "gwsig_exchange_begin": [_vp, _vp, _vp, _vp], "gwsig_exchange_eval": [_vp, _vp, _vp, _vp, _vp],
     "gwsig_p0_begin": [_vp, _vp, _vp, _vp], "gwsig_p0_push_pairs": [_vp, _i64, _i64, _vp], "gwsig_p0_end": [_vp],
     "gwsig_p0_eval": [_vp, _vp, _vp, _vp, _vp], "gwsig_block_transform_v": [_vp, _i64, _i64, _vp, _vp, _vp],
+    "gwsig_dyson_p": [_vp, _vp, _vp, _vp, _i, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -183,7 +184,7 @@ class Gwsig:
         self._ck(_lib.gwsig_last_launch_count(self._h, C.addressof(n)))
         return n.value
 
-    KINDS = ("unfold_G", "unfold_W", "stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV", "epilogue", "vtransform")
+    KINDS = ("unfold_G", "unfold_W", "stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV", "epilogue", "vtransform", "grid_transform", "dyson_solve")
 
     def kernel_times(self):
         ms = np.zeros(len(self.KINDS), np.float64)
@@ -223,6 +224,9 @@ class Gwsig:
 
     def block_transform_v(self, p0, np_, dV_dense, dV_packed, stream=0):
         self._ck(_lib.gwsig_block_transform_v(self._h, p0, np_, _ptr(dV_dense), _ptr(dV_packed), stream or None))
+
+    def dyson_p(self, dP0, dTf, dTb, nw, dP, stream=0):
+        self._ck(_lib.gwsig_dyson_p(self._h, _ptr(dP0), _ptr(dTf), _ptr(dTb), int(nw), _ptr(dP), stream or None))
 
     def p0_begin(self, dG, dP0, stream=0):
         self._ck(_lib.gwsig_p0_begin(self._h, _ptr(dG), _ptr(dP0), stream or None))

@@ -75,6 +75,7 @@ struct gwsig_ctx {
   // device buffers
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
   DevBuf oblk_ao, oblk_aux, unf_tmp, partial;
+  DevBuf dys_flag;                               // N3: singular-matrix flag of the Eq. 19 solve
   DevBuf u_ao_dev, u_aux_dev;                    // N4: the adapted bases on the device (set_blocks with U)
   DevBuf grev, p0acc, p0desc;                    // N1 (Eq. 20): G(beta - tau) on the full zone, the P0 accumulator, its epilogue descriptors
   bool in_p0 = false;
@@ -380,7 +381,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->dys_flag, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -549,7 +550,8 @@ int gwsig_plan_counts(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage,
   const Plan& P = ctx->plan;
   if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_counts: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
+  int rc = stage == 51 ? P.build_gridtransform(P.nk1, (int)np, nt, sp)                          // 51: grid transform, np = n_in, nt = n_out
+         : stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
          : stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
          : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
@@ -565,7 +567,8 @@ int gwsig_plan_get(gwsig_ctx* ctx, int64_t p0, int64_t np, int nt, int stage, vo
   const Plan& P = ctx->plan;
   if (!P.have_sym || (P.v_off.empty() && stage < 30)) return fail(ctx, GWSIG_ERR_ARG, "plan_get: plan incomplete");
   StagePlan sp;
-  int rc = stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
+  int rc = stage == 51 ? P.build_gridtransform(P.nk1, (int)np, nt, sp)                          // 51: grid transform, np = n_in, nt = n_out
+         : stage >= 40 ? P.build_vtransform(p0, np, stage - 40, sp)                             // 41, 42, 43: Eq. 27 steps
          : stage >= 30 ? P.build_p0_stage(p0, np, nt, stage - 30, sp)                           // 31, 32, 33: P0 stages (Eq. 20)
          : stage >= 10 ? P.build_unfold(stage / 10 == 2, (int)p0, (int)np, stage % 10, sp)      // 11, 12: G unfold steps; 21, 22: W
                        : P.build_stage(p0, np, nt, stage, (int)(p0 / P.nk1), sp);
@@ -771,6 +774,63 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
   rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
   if (rc) { ctx->in_eval = false; ctx->exchange = false; return rc; }
   return gwsig_sigma_end(ctx);
+}
+
+/* ---- N3: P^q(tau) from the bare bubble, Eq. 19 ------------------------------------------------------- */
+int gwsig_dyson_p(gwsig_ctx* ctx, const void* dP0, const void* dTf, const void* dTb, int nw, void* dP, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!P.have_sym) return fail(ctx, GWSIG_ERR_ARG, "dyson_p: call set_symmetry first");
+  if (P.mode == GWSIG_IBZ_BLOCK) return fail(ctx, GWSIG_ERR_ARG, "dyson_p: built for the dense layouts (FULL_BZ, IBZ) only");
+  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "dyson_p: an evaluation is open");
+  if (!dP0 || !dTf || !dTb || !dP || nw < 1) return fail(ctx, GWSIG_ERR_ARG, "dyson_p: NULL pointer or nw < 1");
+  if (P.naux > 512) return fail(ctx, GWSIG_ERR_ARG, "dyson_p: naux > 512");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)stream;
+  CU(ctx->counters.ensure(gwsig_ctx::kCounterSlots * sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
+  ctx->counter_slot = 0;
+  ctx->ev_used.clear();
+  ctx->launches = 0;
+  const int nq = P.nk1;
+  const long long n2 = (long long)P.naux * P.naux;
+  const int ncta = 2 * std::max(ctx->num_sms, 1);
+  CU(ctx->xbuf.ensure((size_t)nq * nw * n2 * sizeof(double2)));                       // P0(i Omega), then P(i Omega) in place
+  CU(ctx->ybuf.ensure((size_t)ncta * P.naux * 2 * P.naux * sizeof(double2)));         // per-CTA augmented matrices
+  CU(ctx->dys_flag.ensure(16));
+  CU(cudaMemsetAsync(ctx->dys_flag.p, 0, 16, ctx->stream));
+  auto xform = [&](const double2* src, const double2* T, double2* dst, int nin, int nout) -> int {
+    StagePlan sp;
+    int r = P.build_gridtransform(nq, nin, nout, sp);
+    if (r) return fail(ctx, r, "internal: build_gridtransform failed");
+    DevStage d;
+    d.nprob = (int)sp.prob.size(); d.ntiles = sp.ntiles;
+    if ((r = upload(ctx, d.prob, sp.prob))) return r;
+    if ((r = upload(ctx, d.seg, sp.seg))) return r;
+    if ((r = upload(ctx, d.bucket, sp.bucket))) return r;
+    r = run_stage(ctx, GWSIG_KIND_GRIDXFORM, d, src, T, dst, 0);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    d.prob.release(); d.seg.release(); d.bucket.release();
+    if (r) return r;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "dyson_p transform");
+    return GWSIG_OK;
+  };
+  // P0(i Omega_n) = sum_t Tf[n,t] P0(tau_t)
+  if ((rc = xform((const double2*)dP0, (const double2*)dTf, (double2*)ctx->xbuf.p, P.ntau, nw))) return rc;
+  // P(i Omega) = [1 - P0(i Omega)]^{-1} P0(i Omega)                                   (Eq. 19a)
+  if ((rc = tic(ctx, GWSIG_KIND_DYSON))) return rc;
+  CU(launch_dyson_solve((double2*)ctx->xbuf.p, nq * nw, P.naux, (double2*)ctx->ybuf.p, ncta, (int*)ctx->dys_flag.p, ctx->stream));
+  if ((rc = toc(ctx))) return rc;
+  ctx->launches++;
+  // P(tau_t) = sum_n Tb[t,n] P(i Omega_n)                                             (Eq. 19b)
+  if ((rc = xform((const double2*)ctx->xbuf.p, (const double2*)dTb, (double2*)dP, nw, P.ntau))) return rc;
+  int flag = 0;
+  CU(cudaMemcpyAsync(&flag, ctx->dys_flag.p, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (flag) return fail(ctx, GWSIG_ERR_ARG, "dyson_p: 1 - P0(i Omega) is singular (or an input is not finite) for at least one (q, Omega)");
+  return GWSIG_OK;
 }
 
 /* ---- N4: Eq. 27 on the device --------------------------------------------------------------------------- */

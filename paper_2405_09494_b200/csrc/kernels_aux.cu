@@ -280,6 +280,81 @@ cudaError_t launch_reverse_tau(const double2* src, double2* dst, int nk, int nta
   return cudaGetLastError();
 }
 
+// Eq. 19a: P = [1 - P0]^{-1} P0 for one (q, Omega) per CTA at a time: Gauss-Jordan elimination with partial
+// pivoting on the augmented matrix [1 - P0 | P0] kept in a per-CTA global scratch (L2-resident: 2.9 MB at naux = 300); the pivot
+// row and the factor column of a step sit in shared memory.  2 n^3 complex multiply-adds per matrix: 0.2 % of one pair's
+// contraction, so plain FP64 FMAs.
+constexpr int DYS_NMAX = 512;
+__global__ void __launch_bounds__(256) dyson_solve_kernel(double2* X, int nmat, int n, double2* work, int* fail_flag) {
+  __shared__ double2 prow[2 * DYS_NMAX];
+  __shared__ double2 fac[DYS_NMAX];
+  __shared__ double red_v[256];
+  __shared__ int red_i[256];
+  const int tid = threadIdx.x, nt = blockDim.x, w2 = 2 * n;
+  double2* M = work + (long long)blockIdx.x * n * w2;
+  for (int mat = blockIdx.x; mat < nmat; mat += gridDim.x) {
+    double2* A = X + (long long)mat * n * n;
+    for (int e = tid; e < n * n; e += nt) {
+      const int r = e / n, c = e - r * n;
+      const double2 a = A[e];
+      M[(long long)r * w2 + c] = make_double2((r == c ? 1.0 : 0.0) - a.x, -a.y);
+      M[(long long)r * w2 + n + c] = a;
+    }
+    __syncthreads();
+    for (int c = 0; c < n; ++c) {
+      double best = -1.0; int bi = c;
+      for (int r = c + tid; r < n; r += nt) {
+        const double2 v = M[(long long)r * w2 + c];
+        const double a2 = v.x * v.x + v.y * v.y;
+        if (a2 > best) { best = a2; bi = r; }
+      }
+      red_v[tid] = best; red_i[tid] = bi;
+      __syncthreads();
+      for (int s_ = nt / 2; s_ > 0; s_ >>= 1) {
+        if (tid < s_ && (red_v[tid + s_] > red_v[tid] || (red_v[tid + s_] == red_v[tid] && red_i[tid + s_] < red_i[tid]))) {
+          red_v[tid] = red_v[tid + s_]; red_i[tid] = red_i[tid + s_];
+        }
+        __syncthreads();
+      }
+      const int piv = red_i[0];
+      const double pv2 = red_v[0];
+      if (pv2 <= 0.0 || !(pv2 == pv2)) { if (tid == 0) *fail_flag = 1; }           // singular 1 - P0 (or NaN input): flagged, result undefined
+      const double2 pv = M[(long long)piv * w2 + c];
+      __syncthreads();
+      const double inv_r = pv.x / pv2, inv_i = -pv.y / pv2;                          // 1 / pivot
+      // swap rows c <-> piv on columns c .. 2n-1 while scaling the pivot row; keep it in shared memory
+      for (int j = c + tid; j < w2; j += nt) {
+        const double2 a = M[(long long)piv * w2 + j], b = M[(long long)c * w2 + j];
+        const double2 sc = make_double2(a.x * inv_r - a.y * inv_i, a.x * inv_i + a.y * inv_r);
+        if (piv != c) M[(long long)piv * w2 + j] = b;
+        M[(long long)c * w2 + j] = sc;
+        prow[j] = sc;
+      }
+      __syncthreads();
+      for (int r = tid; r < n; r += nt) fac[r] = r == c ? make_double2(0.0, 0.0) : M[(long long)r * w2 + c];
+      __syncthreads();
+      const int wj = w2 - (c + 1);
+      for (long long e = tid; e < (long long)n * wj; e += nt) {
+        const int r = (int)(e / wj), j = c + 1 + (int)(e - (long long)r * wj);
+        const double2 f = fac[r], pr = prow[j];
+        double2* d = &M[(long long)r * w2 + j];
+        d->x -= f.x * pr.x - f.y * pr.y;
+        d->y -= f.x * pr.y + f.y * pr.x;
+      }
+      __syncthreads();
+    }
+    for (int e = tid; e < n * n; e += nt) A[e] = M[(long long)(e / n) * w2 + n + (e % n)];
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_dyson_solve(double2* X, int nmat, int n, double2* work, int ncta, int* fail_flag, cudaStream_t stream) {
+  if (nmat <= 0) return cudaSuccess;
+  if (n > DYS_NMAX || ncta < 1) return cudaErrorInvalidValue;
+  dyson_solve_kernel<<<(unsigned)std::min(ncta, nmat), 256, 0, stream>>>(X, nmat, n, work, fail_flag);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream) {
   if (ngroups <= 0) return cudaSuccess;
   for (int g0 = 0; g0 < ngroups; g0 += 65535) {

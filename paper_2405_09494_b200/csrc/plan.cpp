@@ -818,6 +818,38 @@ int Plan::build_vtransform(long long p0, long long np, int step, StagePlan& out)
   return GWSIG_OK;
 }
 
+int Plan::build_gridtransform(int nq, int nin, int nout, StagePlan& out) const {
+  out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
+  if (nq < 1 || nin < 1 || nout < 1) return GWSIG_ERR_ARG;
+  const long long n2 = (long long)naux * naux;
+  if (n2 >= (1LL << 31)) return GWSIG_ERR_ARG;
+  long long tb = 0;
+  for (int q = 0; q < nq; ++q) {
+    gwsig_seg S; std::memset(&S, 0, sizeof(S));
+    gwsig_problem P; std::memset(&P, 0, sizeof(P));
+    S.a_off = (long long)q * nin * n2; S.am = lvl1(1); S.ak = lvl1(n2);       // A[m, i] = src[q][i][m]
+    S.b_off = 0; S.bk = lvl1(1); S.bn = lvl1(nin);                            // B[i, o] = T[o][i]
+    S.K = nin;
+    P.M = (int)n2; P.N = nout;
+    P.c_off = (long long)q * nout * n2; P.cm = lvl1(1); P.cn = lvl1(n2);      // C[m, o] = dst[q][o][m]
+    P.nbatch = 1; P.flags = 0;
+    P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+    P.tiles_m = zg_tiles_m(P.M, tile_m[0]); P.tiles_n = zg_tiles_n(P.N);
+    P.tile_begin = tb;
+    tb += (long long)P.tiles_m * P.tiles_n;
+    out.seg.push_back(S); out.prob.push_back(P);
+  }
+  out.ntiles = tb;
+  out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
+  size_t pi = 0;
+  for (size_t bkt = 0; bkt < out.bucket.size(); ++bkt) {
+    const long long t = (long long)bkt << ZG_BUCKET_SHIFT;
+    while (pi + 1 < out.prob.size() && out.prob[pi + 1].tile_begin <= t) ++pi;
+    out.bucket[bkt] = (int)pi;
+  }
+  return GWSIG_OK;
+}
+
 int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePlan& out, int num_sms) const {
   out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
   if (mode == GWSIG_IBZ_BLOCK) return GWSIG_ERR_ARG;                // dense modes only

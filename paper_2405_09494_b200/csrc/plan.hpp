@@ -144,6 +144,8 @@ struct Plan {
   //   step 3  packed(P,a,i) = sum_j T2[P][a][j] U^{k1}[j,i]   for the allowed triples only, written in the packed layout
   // A: dense V2 / T1 / T2 (pair l at l * naux * nao^2), B: the U_aux table (step 1) or the U_ao table (steps 2, 3), [Nk][n][n]
   int build_vtransform(long long p0, long long np, int step, StagePlan& out) const;
+  // ---- N3 (Eq. 19): dst[q][o][m] = sum_i T[o][i] src[q][i][m] for nq momenta, m over naux^2 (tau <-> i Omega transforms as GEMMs)
+  int build_gridtransform(int nq, int nin, int nout, StagePlan& out) const;
   int build_p0_stage(long long p0, long long np, int nt, int stage, StagePlan& out, int num_sms = 148) const;
 };
 

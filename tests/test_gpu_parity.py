@@ -354,6 +354,47 @@ def test_block_transform_v_eq27(name):
     _check(cfg, inp, run_gpu(cfg, G, W, got), ks=None if inp.nk <= 64 else list(range(0, inp.nk, 7)))
 
 
+@pytest.mark.parametrize("name,mode,nw", [("toy_wurtzite", 1, 3), ("cfg2", 1, 9), ("cfg1", 0, 7)])
+def test_dyson_p_eq19(name, mode, nw):
+    """N3: P = [1 - P0]^{-1} P0 per (q, Omega) with caller-supplied tau <-> i Omega transform matrices (Eq. 19)
+    through gwsig_dyson_p against oracle/dyson_oracle.py; the input P0 is the oracle's own bare bubble, scaled to |P0| ~ 1 so that
+    the solve is far from the perturbative regime; a singular 1 - P0 is reported."""
+    B = _B()
+    torch = _torch()
+    from oracle.dyson_oracle import dyson_p_ref
+    from paper_2405_09494_b200.pack import Configured, configure_from_crystal
+    lib = B.Gwsig(device=0)
+    if name == "cfg1":
+        inp = get_inputs("cfg1")
+        cfg = Configured(lib, mode, np.eye(3), inp.kmesh.N, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
+    else:
+        inp = get_inputs(name)
+        cfg = configure_from_crystal(lib, inp.cr, mode)
+    qs = list(cfg.out_list)[:6]
+    lib.set_output_points(qs) if len(qs) < len(cfg.out_list) else None
+    P0 = oracle_p0(inp, qs)
+    P0 = P0 / np.abs(P0).max() * 0.9
+    rng = np.random.default_rng(3)
+    tau = np.arange(inp.ntau) * inp.beta / (inp.ntau - 1)
+    om = 2 * np.pi * np.arange(nw) / inp.beta
+    Tf = np.exp(1j * np.outer(om, tau)) * (inp.beta / inp.ntau) + 0.01 * rng.standard_normal((nw, inp.ntau))     # a quadrature-like matrix
+    Tb = np.exp(-1j * np.outer(tau, om)) / inp.beta
+    ref = dyson_p_ref(P0, Tf, Tb)
+    dP0, dTf, dTb = (torch.from_numpy(np.ascontiguousarray(x, np.complex128)).cuda() for x in (P0, Tf, Tb))
+    dP = torch.full((P0.size,), float("nan"), dtype=torch.complex128, device="cuda")
+    lib.dyson_p(dP0, dTf, dTb, nw, dP, torch.cuda.current_stream().cuda_stream)
+    got = dP.cpu().numpy().reshape(P0.shape)
+    worst = max(rel_err(got[i, t], ref[i, t]) for i in range(len(qs)) for t in range(inp.ntau))
+    cond = max(np.linalg.cond(np.eye(inp.naux) - np.einsum("wt,tab->wab", Tf, P0[i])).max() for i in range(len(qs)))
+    assert worst <= max(TOL, 1e-15 * cond * 100), (worst, cond)
+    # singular case: P0(i Omega) = 1 exactly for identity transforms
+    if name == "cfg1":
+        one = np.tile(np.eye(inp.naux, dtype=complex), (len(qs), inp.ntau, 1, 1))
+        eye = torch.eye(inp.ntau, dtype=torch.complex128, device="cuda")
+        with pytest.raises(B.GwsigError):
+            lib.dyson_p(torch.from_numpy(one).cuda(), eye, eye, inp.ntau, dP, 0)
+
+
 def test_output_point_subset_matches_full_run():
     B, inp, cfg, G, W, V = _setup("toy_diamond", 2)
     full = cfg.unpack_sigma(run_gpu(cfg, G, W, V))

@@ -248,3 +248,20 @@ def test_vtransform_plan_matches_oracle(name):
     assert got.shape == ref.shape and np.abs(got - ref).max() < 1e-13 * np.abs(ref).max()
     with pytest.raises(B.GwsigError):                      # S5 gauge recognised: the Eq. 28 unfold stages are not available
         lib.plan_get(0, 4, inp.ntau, 11)
+
+
+def test_gridtransform_plan_matches_einsum():
+    """N3 (Eq. 19): the tau <-> i Omega transform descriptors (plan stage 51), run by the numpy interpreter, are the einsum."""
+    from tests.helpers import run_stage_numpy
+    inp = make_inputs("toy_sc")
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ)
+    nq, n2, nin, nout = cfg.nk1, inp.naux ** 2, inp.ntau, 5
+    rng = np.random.default_rng(1)
+    src = rng.standard_normal(nq * nin * n2) + 1j * rng.standard_normal(nq * nin * n2)
+    T = rng.standard_normal((nout, nin)) + 1j * rng.standard_normal((nout, nin))
+    pr, sg, _ = lib.plan_get(0, nin, nout, 51)
+    dst = np.zeros(nq * nout * n2, complex)
+    run_stage_numpy(pr, sg, src, T.ravel(), dst, 0)
+    want = np.einsum("oi,qim->qom", T, src.reshape(nq, nin, n2))
+    assert np.abs(dst.reshape(nq, nout, n2) - want).max() < 1e-13
