@@ -46,101 +46,6 @@ __global__ void __launch_bounds__(256) unfold_sparse_kernel(UnfoldParams p) {
   p.dst[((long long)tgt * p.ntau + t) * n * n + e] = make_double2(sr, si);
 }
 
-// Tiled version of the same product, used when a row tile's source rows fit the shared-memory panel (always, for shell-
-// structured representations): one CTA = (target k', tau, tile of UNF_RB output rows).
-//   step A  T[s, c] = sum_{n in nz(c)} X[m_s, n] P[c, n] conj(ph[n])   for the source rows m_s the tile needs, all columns c
-//   step B  out[r, c] = sum_{m in nz(r)} P[r, m] ph[m] T[pos(m), c]
-// X rows are read with consecutive threads on consecutive columns (the gathers of neighbouring columns hit the same lines),
-// T lives in shared memory, the output is written once with full lines: the kernel is bound by that write (HBM).
-constexpr int UNF_RB = 8;         // output rows per CTA
-constexpr int UNF_NS = 32;        // source-row panel (rows of T); a tile that needs more falls back to the element-wise path
-__global__ void __launch_bounds__(256) unfold_tiled_kernel(UnfoldParams p) {
-  extern __shared__ double2 unf_T[];                 // [UNF_NS][n]
-  __shared__ int need[512];                          // n <= 512: position of source row m in the panel, or -1
-  __shared__ int srow[UNF_NS];
-  __shared__ int ns_sh;
-  const int n = p.n;
-  const int tgt = blockIdx.x / p.ntau, t = blockIdx.x % p.ntau;
-  const int r0 = blockIdx.y * UNF_RB, nrow = min(UNF_RB, n - r0);
-  const int op = p.tgt_op[tgt];
-  const double2* X = p.src + ((long long)p.tgt_src[tgt] * p.ntau + t) * n * n;
-  const double2* ph = p.colphase + (long long)tgt * n;
-  double2* out = p.dst + ((long long)tgt * p.ntau + t) * n * n;
-  const int* ecols = p.ell_cols + (long long)op * n * p.maxnz;
-  const double* evals = p.ell_vals + (long long)op * n * p.maxnz;
-  const int* ecnt = p.ell_cnt + op * n;
-  for (int i = threadIdx.x; i < n; i += blockDim.x) need[i] = -1;
-  __syncthreads();
-  for (int i = threadIdx.x; i < nrow * p.maxnz; i += blockDim.x) {
-    const int r = r0 + i / p.maxnz, a = i % p.maxnz;
-    if (a < ecnt[r]) need[ecols[(long long)r * p.maxnz + a]] = 0;
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {                            // compact the (few) needed source rows
-    int ns = 0;
-    for (int m = 0; m < n; ++m)
-      if (need[m] == 0) { if (ns < UNF_NS) srow[ns] = m; need[m] = ns < UNF_NS ? ns : -2; ++ns; }
-    ns_sh = ns;
-  }
-  __syncthreads();
-  const int ns = ns_sh;
-  if (ns > UNF_NS) {
-    // fallback: element-wise double sum for this tile (never taken for perm (x) Wigner-D representations with RB = 8)
-    for (int e = threadIdx.x; e < nrow * n; e += blockDim.x) {
-      const int r = r0 + e / n, c = e % n;
-      double sr = 0.0, si = 0.0;
-      for (int a = 0; a < ecnt[r]; ++a) {
-        const int m = ecols[(long long)r * p.maxnz + a];
-        const double2 pm = ph[m];
-        const double wr = evals[(long long)r * p.maxnz + a] * pm.x, wi = evals[(long long)r * p.maxnz + a] * pm.y;
-        double tr = 0.0, ti = 0.0;
-        for (int b = 0; b < ecnt[c]; ++b) {
-          const int nn = ecols[(long long)c * p.maxnz + b];
-          const double2 x = X[(long long)m * n + nn];
-          const double2 pn = ph[nn];
-          const double ur = evals[(long long)c * p.maxnz + b] * pn.x, ui = -evals[(long long)c * p.maxnz + b] * pn.y;
-          tr += x.x * ur - x.y * ui; ti += x.x * ui + x.y * ur;
-        }
-        sr += wr * tr - wi * ti; si += wr * ti + wi * tr;
-      }
-      out[(long long)r * n + c] = make_double2(sr, si);
-    }
-    return;
-  }
-  // step A
-  for (int e = threadIdx.x; e < ns * n; e += blockDim.x) {
-    const int s_ = e / n, c = e - s_ * n;
-    const double2* xr = X + (long long)srow[s_] * n;
-    double tr = 0.0, ti = 0.0;
-    const int nc = ecnt[c];
-    for (int b = 0; b < nc; ++b) {
-      const int nn = ecols[(long long)c * p.maxnz + b];
-      const double v = evals[(long long)c * p.maxnz + b];
-      const double2 x = xr[nn];
-      const double2 pn = ph[nn];
-      const double ur = v * pn.x, ui = -v * pn.y;
-      tr += x.x * ur - x.y * ui; ti += x.x * ui + x.y * ur;
-    }
-    unf_T[e] = make_double2(tr, ti);
-  }
-  __syncthreads();
-  // step B
-  for (int e = threadIdx.x; e < nrow * n; e += blockDim.x) {
-    const int rr = e / n, c = e - rr * n, r = r0 + rr;
-    double sr = 0.0, si = 0.0;
-    const int nr = ecnt[r];
-    for (int a = 0; a < nr; ++a) {
-      const int m = ecols[(long long)r * p.maxnz + a];
-      const double v = evals[(long long)r * p.maxnz + a];
-      const double2 pm = ph[m];
-      const double wr = v * pm.x, wi = v * pm.y;
-      const double2 tv = unf_T[need[m] * n + c];
-      sr += wr * tv.x - wi * tv.y; si += wr * tv.y + wi * tv.x;
-    }
-    out[(long long)r * n + c] = make_double2(sr, si);
-  }
-}
-
 // Sigma = scale * acc, optionally (Sigma + Sigma^dagger)/2, for a list of square-matrix batches.
 __global__ void __launch_bounds__(256) epilogue_kernel(EpilogueParams p) {
   const int d = blockIdx.y;
@@ -245,22 +150,6 @@ __global__ void probe_mixed_kernel(long long iters, double* sink) {
 
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream) {
   if (ntarget <= 0) return cudaSuccess;
-  constexpr int kMaxDyn = 227 * 1024 - 4096;                         // opt-in limit minus the kernel's static shared memory
-  const int smem = UNF_NS * p.n * (int)sizeof(double2);              // 154 KB at naux = 300
-  if (p.n <= 512 && smem <= kMaxDyn) {
-    static bool attr_set[64] = {false};
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-      e = cudaFuncSetAttribute(unfold_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDyn);
-      if (e != cudaSuccess) return e;
-      attr_set[dev] = true;
-    }
-    dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n + UNF_RB - 1) / UNF_RB));
-    unfold_tiled_kernel<<<grid, 256, smem, stream>>>(p);
-    return cudaGetLastError();
-  }
   dim3 grid((unsigned)((long long)ntarget * p.ntau), (unsigned)((p.n * p.n + 255) / 256));
   unfold_sparse_kernel<<<grid, 256, 0, stream>>>(p);
   return cudaGetLastError();
