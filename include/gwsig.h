@@ -190,6 +190,28 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
  * 1 - P0(i Omega) is singular.                                                                                       */
 int gwsig_dyson_p(gwsig_ctx* ctx, const void* dP0, const void* dTf, const void* dTb, int nw, void* dP, void* stream);
 
+/* ---- the Eq. 19a solve for callers that may not allocate -------------------------------------------------------------
+ * X_m = [1 - A_m]^{-1} A_m for m < nmat (Eq. 19a: P(q, i Omega) from P0(q, i Omega); one matrix per (q, Omega)).
+ * Code under CUDA graph capture, tight serving loops and harnesses that forbid cudaMalloc cannot use gwsig_dyson_p, whose
+ * context grows its buffers on demand.  This entry point takes no context, calls no cudaMalloc / cudaFree and no allocating
+ * library routine, and does not synchronise: it clears *d_info and launches ONE kernel on `stream`.  Its scratch (one
+ * augmented matrix [n][2n] per CTA) is a file-scope `static __device__` array of GWSIG_NOALLOC_SCRATCH_BYTES that every GPU
+ * which loads the library holds until the process exits; the first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress: no allocation, but make that first call outside stream capture).
+ *   dA (dev, in)  [nmat][n][n] complex128 row-major, caller-owned, not modified unless dX == dA
+ *   dX (dev, out) same shape; dX == dA (in place) is allowed, partial overlap is not
+ *   d_info (dev, out, may be NULL) one int: 0, or 1 if some 1 - A_m was singular / not finite (that X_m is then undefined)
+ *   stream: a stream of the CURRENT device (the caller's inputs live there); the call returns once the work is queued
+ * n <= GWSIG_NOALLOC_NMAX, else GWSIG_ERR_ARG; nmat is unbounded (CTAs loop over the matrices).  ALL calls of a device share
+ * the one scratch array: calls that can overlap on the GPU (different streams, or graph branches without an edge between
+ * them) race -- order them on one stream or with events.  The scratch keeps the last call's contents; nothing in it has to
+ * start at zero (every element read was written by the same matrix' pass).  Same elimination, pivoting rule and operation
+ * order as the kernel behind gwsig_dyson_p.  On error returns GWSIG_ERR_ARG / GWSIG_ERR_CUDA and, when errbuf != NULL,
+ * writes a NUL-terminated message of at most errbuf_len bytes (host).                                                    */
+#define GWSIG_NOALLOC_NMAX 256
+#define GWSIG_NOALLOC_SCRATCH_BYTES (16 << 20)
+int gwsig_dyson_solve_noalloc(const void* dA, void* dX, int nmat, int n, void* d_info, void* stream, char* errbuf, int errbuf_len);
+
 /* ---- N4: block-basis transform of V on the device ----------------------------------------
  * V2blk_{P,a,i} = sum_{Q,b,j} conj(Uaux^q_{Q,P}) conj(U^{k2}_{b,a}) V2_{Q,b,j} U^{k1}_{j,i}     (Eq. 27; V2 = V^{k2,k1},
  * q = k1 - k2) for pairs p0 .. p0+np-1: dV_dense (dev) holds the orbital-basis tensors [naux][nao][nao] back to back in pair

@@ -36,7 +36,8 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_sigma_eval", "gwsig_set_option", "gwsig_flop_counts", "gwsig_last_launch_count", "gwsig_plan_counts",
            "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host",
            "gwsig_set_output_points", "gwsig_exchange_begin", "gwsig_exchange_eval",
-           "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval", "gwsig_block_transform_v", "gwsig_dyson_p"]
+           "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval", "gwsig_block_transform_v", "gwsig_dyson_p",
+           "gwsig_dyson_solve_noalloc"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -56,6 +57,7 @@ _sig = {
     "gwsig_p0_begin": [_vp, _vp, _vp, _vp], "gwsig_p0_push_pairs": [_vp, _i64, _i64, _vp], "gwsig_p0_end": [_vp],
     "gwsig_p0_eval": [_vp, _vp, _vp, _vp, _vp], "gwsig_block_transform_v": [_vp, _i64, _i64, _vp, _vp, _vp],
     "gwsig_dyson_p": [_vp, _vp, _vp, _vp, _i, _vp, _vp],
+    "gwsig_dyson_solve_noalloc": [_vp, _vp, _i, _i, _vp, _vp, C.c_char_p, _i],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -83,6 +85,18 @@ def _ptr(x):
 
 def _np(x, dtype):
     return np.ascontiguousarray(x, dtype=dtype)
+
+
+NOALLOC_NMAX, NOALLOC_SCRATCH_BYTES = 256, 16 << 20
+
+
+def dyson_solve_noalloc(dA, dX, nmat, n, d_info=None, stream=0):
+    """gwsig_dyson_solve_noalloc: X_m = [1 - A_m]^{-1} A_m (Eq. 19a) with the library's fixed device scratch; takes no
+    context, allocates nothing, does not synchronise.  dA / dX: device complex128 [nmat][n][n]; d_info: device int32 or None."""
+    err = C.create_string_buffer(256)
+    rc = _lib.gwsig_dyson_solve_noalloc(_ptr(dA), _ptr(dX), int(nmat), int(n), _ptr(d_info), stream or None, err, len(err))
+    if rc:
+        raise GwsigError(rc, err.value.decode())
 
 
 class Gwsig:

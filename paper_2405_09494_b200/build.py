@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgwsig.so")
-SOURCES = ["gwsig.cu", "plan.cpp", "zgemm_grouped.cu", "kernels_aux.cu"]
+SOURCES = ["gwsig.cu", "plan.cpp", "zgemm_grouped.cu", "kernels_aux.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O3", "-shared", "-cudart", "static"]
 
