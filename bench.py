@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--ibz-nq", type=int, default=0, help="q slices timed in the IBZ comparison leg (0: all; 16 at cfg4/cfg5), scaled")
     ap.add_argument("--full-nq", type=int, default=0, help="q slices timed in the FULL_BZ comparison leg (0: 8; 2 at cfg4/cfg5), scaled")
     ap.add_argument("--engine", type=int, default=0, choices=[0, 2, 3], help="0: per-stage choice (default), 2: DMMA 4M kernel, 3: DMMA 3M kernel")
+    ap.add_argument("--scratch-mib", type=int, default=0, help="main leg only: cap of the X + Y scratch in MiB (0: library default, 8192); small values "
+                    "give chunks that stay in L2 at the price of many short launches (experiments)")
     ap.add_argument("--probe-only", action="store_true", help="print the FP64 issue-rate probes and exit")
     return ap.parse_args()
 
@@ -541,6 +543,8 @@ def main():
     wl = Workload(args.workload, mode, B, pack, torch=torch, dev=dev, device_index=local)
     cfg, lib = wl.cfg, wl.lib
     lib.set_option("engine", args.engine)
+    if args.scratch_mib > 0:
+        lib.set_option("scratch_mib", args.scratch_mib)
     t_setup = time.time() - t_setup
 
     # ---- the timed region: W warm-up steps, then exactly K steps between barrier + synchronize --------------
@@ -575,7 +579,7 @@ def main():
     line = {"metric": METRIC, "value": ms_eval, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex128 (f64)", "data": "synthetic",
-            "config": {"workload": f"{args.workload} ({describe(args.workload)})", "mode": args.mode, "engine": {0: "dmma (3M stage 2, 4M stages 1 and 3)", 2: "dmma 4M", 3: "dmma 3M"}[args.engine], "nk": int(cfg.nk), "nik": int(cfg.nk1),
+            "config": {"workload": f"{args.workload} ({describe(args.workload)})", "mode": args.mode, "engine": {0: "dmma (3M stages 1 and 2, 4M stage 3)", 2: "dmma 4M", 3: "dmma 3M"}[args.engine], "nk": int(cfg.nk), "nik": int(cfg.nk1),
                        "nao": int(cfg.nao), "naux": int(cfg.naux), "ntau": int(cfg.ntau), "pairs": int(cfg.npairs),
                        "l2": "inputs larger than L2 (V alone is %.2f GB)" % (wl.setup_notes.get("v_total_gb") or wl.V.nbytes / 1e9),
                        "v": ("resident in HBM" if wl.resident else "synthesised on the device per batch of whole q INSIDE the step (all pairs do not fit HBM): "
@@ -605,7 +609,7 @@ def main():
     probe_tf = max(lib.probe_fp64(0, w, b, 20000)[0] for w, b in ((8, 2), (16, 2)))
     dom = int(np.argmax([t1, t2, t3]))
     ach = sf[dom] / max((t1, t2, t3)[dom], 1e-12) / 1e12
-    line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + (" (zgemm_grouped_dmma3m)" if (args.engine == 3 or (args.engine == 0 and dom == 1)) else " (zgemm_grouped_dmma)"),
+    line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + (" (zgemm_grouped_dmma3m)" if (args.engine == 3 or (args.engine == 0 and dom in (0, 1))) else " (zgemm_grouped_dmma)"),
                         "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
                         "peak_measured_dmma_probe": probe_tf,
                         "peak_source": "FP64 tensor (DMMA) peak derived from unit counts x max clock, 148 x 128 flop/clk x 1.965 GHz "

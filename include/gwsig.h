@@ -48,7 +48,7 @@ typedef enum {
 
 typedef enum {
   GWSIG_ENGINE_DMMA = 0,      /* FP64 tensor-core grouped GEMM (mma.sync m8n8k4 f64 -> DMMA), default: per stage the
-                                 faster of the two tensor kernels below (3M for stage 2, 4M for stages 1 and 3)         */
+                                 faster of the two tensor kernels below (3M for stages 1 and 2, 4M for stage 3)         */
   GWSIG_ENGINE_REFERENCE = 1, /* one-thread-per-element DFMA kernels on the same plan (debug)                       */
   GWSIG_ENGINE_DMMA_4M = 2,   /* every stage on the tensor-core kernel with the conventional 4-product complex multiply */
   GWSIG_ENGINE_DMMA_3M = 3    /* every stage on the tensor-core kernel with the 3M / Karatsuba complex multiply:

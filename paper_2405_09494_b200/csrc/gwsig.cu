@@ -287,10 +287,10 @@ int toc(gwsig_ctx* ctx) {
 }
 
 // which kernel runs launch kind st (0 = Eq. 28 unfold, 1..3 = contraction stage) under engine option e:
-// GWSIG_ENGINE_DMMA (default) = the 3M kernel where it is the faster one on B200 (stage 2, 70 % of the flops: K = n_p up to
-// 116) and the 4-product kernel for the short-K stage 1, the narrow-N stage 3 and the unfold (measured)
+// GWSIG_ENGINE_DMMA (default) = the 3M kernel where it is the faster one on B200 (stages 1 and 2: 86 % of the flops) and the
+// 4-product kernel for stage 3 (two-level k index, narrow N, atomic accumulation) and the unfold (measured)
 int stage_engine(int e, int st) {
-  if (e == GWSIG_ENGINE_DMMA) return st == 2 ? GWSIG_ENGINE_DMMA_3M : GWSIG_ENGINE_DMMA_4M;
+  if (e == GWSIG_ENGINE_DMMA) return (st == 1 || st == 2) ? GWSIG_ENGINE_DMMA_3M : GWSIG_ENGINE_DMMA_4M;
   return e;
 }
 void set_tile_heights(gwsig_ctx* ctx) {

@@ -341,6 +341,17 @@ void Plan::w_source(int q, int q_first, long long& off, long long& tstride) cons
 static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo; d.div = GWSIG_NODIV; d.pad_ = 0; return d; }
 static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
 
+// the tensor kernels' epilogues keep the element offset of a tile COLUMN (relative to the tile's C base) in 32 bits
+static bool col_offsets_fit(const std::vector<gwsig_problem>& prob) {
+  for (const auto& P : prob) {
+    if (P.N <= 0) continue;
+    const long long n = P.N - 1;
+    const long long off = P.cn.div == GWSIG_NODIV ? n * P.cn.lo : (n / P.cn.div) * P.cn.hi + std::min<long long>(P.cn.div - 1, n) * P.cn.lo;
+    if (off < 0 || off >= (1LL << 31)) return false;
+  }
+  return true;
+}
+
 int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first, StagePlan& out, int num_sms) const {
   out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
   if (p0 < 0 || np < 1 || p0 + np > npairs || nt < 1 || nt > ntau || stage < 1 || stage > 3) return GWSIG_ERR_ARG;
@@ -586,6 +597,7 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
     sorted[i] = P;
   }
   out.prob.swap(sorted);
+  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   {
@@ -724,6 +736,7 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
   }
+  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -807,6 +820,7 @@ int Plan::build_vtransform(long long p0, long long np, int step, StagePlan& out)
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
   }
+  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -839,6 +853,7 @@ int Plan::build_gridtransform(int nq, int nin, int nout, StagePlan& out) const {
     tb += (long long)P.tiles_m * P.tiles_n;
     out.seg.push_back(S); out.prob.push_back(P);
   }
+  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -942,6 +957,7 @@ int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePla
     sorted[i] = P;
   }
   out.prob.swap(sorted);
+  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;

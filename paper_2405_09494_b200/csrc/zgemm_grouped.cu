@@ -86,8 +86,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 __device__ __forceinline__ double xor_hi(double x, unsigned m) {      // sign flips on the integer pipe
   return __hiloint2double(__double2hiint(x) ^ (int)m, __double2loint(x));
 }
+// Column map of the B fragment.  A DMMA hands lane (fr, fk) the accumulator columns 2 fk, 2 fk + 1 of an 8-column group; were
+// those the tile's columns 2 fk, 2 fk + 1, one store instruction (fixed c) would write 16-byte pieces 32 bytes apart: half
+// sectors, twice the L2 write slots of the payload.  The lane that feeds B column n of the group therefore loads TILE column
+// zg_bcol(n), so that accumulator column 2 fk is tile column fk and 2 fk + 1 is tile column 4 + ((fk + 1) & 3): a store
+// instruction then covers four adjacent complex numbers (64 contiguous bytes) per row.  (The odd distance between the tile
+// columns of a lane pair keeps the 16-byte fragment loads bank-conflict free with LDB = 2 mod 8.)
+__device__ __forceinline__ int zg_bcol(int n) { return (n & 1) ? 4 + (((n >> 1) + 1) & 3) : (n >> 1); }
+__device__ __forceinline__ int zg_ccol(int fk, int c) { return c ? 4 + ((fk + 1) & 3) : fk; }     // tile column (within the group) of accumulator c
+
 __device__ __forceinline__ void red_add(double* addr, double v) {
   asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(addr), "d"(v) : "memory");
+}
+__device__ __forceinline__ void st_pred(double2* addr, double re, double im, bool on) {      // predicated 16-byte store: no branch
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\t@q st.global.v2.f64 [%0], {%1, %2};\n\t}\n" ::"l"(addr), "d"(re), "d"(im), "r"((int)on)
+               : "memory");
 }
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
@@ -309,7 +322,7 @@ __device__ __forceinline__ void consume_slot(double (&acc)[4][4][4], const doubl
   for (int kk = 0; kk < nk4; ++kk) consume_k4<MI, NI>(acc, as + kk * 4 * LDA, bs + kk * 4 * LDB, mask_n, mask_y, mask_b);
 }
 
-// registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + 2 fk + c of the tile.
+// registers -> C (two-level addressing); rows (warp + 4 i) * 8 + fr, columns j * 8 + zg_ccol(fk, c) of the tile.
 // One instance for all variants (bounds are run-time, accumulator indices compile-time).  Lane L computes the offset of
 // tile column L and of the warp's L-th row once; the lanes then fetch the ones they need by shuffle (one idx2 site each).
 __device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const TileRec& t, double2* C, int warp, int lane) {
@@ -324,7 +337,7 @@ __device__ __forceinline__ void store_tile(const double (&acc)[4][4][4], const T
 #pragma unroll
   for (int j = 0; j < 4; ++j)
 #pragma unroll
-    for (int c = 0; c < 2; ++c) coff[j][c] = __shfl_sync(0xffffffffu, my_col, j * 8 + fk * 2 + c);
+    for (int c = 0; c < 2; ++c) coff[j][c] = __shfl_sync(0xffffffffu, my_col, j * 8 + zg_ccol(fk, c));
 #pragma unroll
   for (int i = 0; i < 4; ++i) roff[i] = __shfl_sync(0xffffffffu, my_row, i * 8 + fr);
 #pragma unroll
@@ -413,7 +426,7 @@ __global__ void __launch_bounds__((kConsumerWarps + kProducerWarps) * 32, 2) zge
       }
       if (variant >= 0) {
         const double2* as = As + stage * BK * LDA + fk * LDA + warp * 8 + fr;
-        const double2* bs = Bs + stage * BK * LDB + fk * LDB + fr;
+        const double2* bs = Bs + stage * BK * LDB + fk * LDB + zg_bcol(fr);
         const int nk4 = hdr[stage].nk4;
 #define ZG_F(MI_, NI_) consume_slot<MI_, NI_>(acc, as, bs, nk4, mask_n, mask_y, mask_b);
         switch (variant) { ZG_VARIANTS(ZG_F) default: break; }
@@ -495,6 +508,7 @@ __device__ __forceinline__ void cp_async16_sz(unsigned smem_dst, const void* gme
 // arithmetic.  Operands move as one 16-byte cp.async per element, lane <-> tile row / column (tile rows lane, lane + 32);
 // with ZgParams::use_bulk an operand whose tile dimension is ONE contiguous run (single-level index with unit stride: X / Y
 // and W rows in stage 2, V2 rows in stage 3) moves as one bulk copy per k-row instead, issued by lane 0 (UBLKCP).
+template <bool kBulk>
 __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2* Bs, unsigned full0, unsigned empty0, SlotHdr* hdr,
                                         TileRec* trec, long long* next_tile, int lw, int lane) {
   const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
@@ -533,7 +547,7 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
         const int nslots = (K + BK3 - 1) / BK3;
         const int j0 = (lw - gslot + kLoaderWarps3) % kLoaderWarps3;       // this warp's first slot of the segment
         if (j0 < nslots) {
-          const bool a_row = p.use_bulk && S.am.div == GWSIG_NODIV && S.am.lo == 1, b_row = p.use_bulk && S.bn.div == GWSIG_NODIV && S.bn.lo == 1;
+          const bool a_row = kBulk && S.am.div == GWSIG_NODIV && S.am.lo == 1, b_row = kBulk && S.bn.div == GWSIG_NODIV && S.bn.lo == 1;
           const double2* abase = p.A + __ldg(&S.a_off) + a_boff + (a_row ? m0 : 0);
           const double2* bbase = p.B + __ldg(&S.b_off) + b_boff + (b_row ? n0 : 0);
           // per-lane source pointers of tile rows lane, lane + 32 and tile column lane; lanes outside the tile point at the
@@ -673,28 +687,44 @@ __device__ __forceinline__ void mma3_slot(double (&acc)[4][3][2], const double2*
   }
 }
 
-// accumulators of one row group -> C: re = P1 - P2, im = P3 - P1 - P2; lane (fr, fk) holds row fr, columns 8 j + 2 fk + c
+// accumulators of one row group -> C: re = P1 - P2, im = P3 - P1 - P2; lane (fr, fk) holds row fr, columns 8 j + zg_ccol(fk, c).
+// Lane L computes the offset of tile column L once (32 bits: checked by the plan); the eight shuffles that hand every lane
+// its own column offsets are issued back to back, and the stores carry no branch but their own predicate: with K = n_alpha
+// <= 26 in stage 1 a tile is two slots of DMMA work, and this epilogue is what the MMA warps spend the rest of their time in.
 __device__ __forceinline__ void store_rows3(const double (&acc)[4][3][2], const TileRec& t, double2* C, int rg, int lane) {
   const int fr = lane >> 2, fk = lane & 3;
-  double2* cbase = C + t.c_off;
-  const bool accum = (t.flags & GWSIG_FLAG_ACCUM) != 0;
-  const long long my_col = lane < t.ncols ? idx2(t.cn, t.n0 + lane) : -1;
+  const int ncols = t.ncols;
+  const int my_col = lane < ncols ? (int)idx2(t.cn, t.n0 + lane) : 0;
   const int row = rg * 8 + fr;
-  const long long roff = row < t.mrows ? idx2(t.cm, t.m0 + row) : -1;
+  const bool rok = row < t.mrows;
+  double2* rowp = C + t.c_off + (rok ? idx2(t.cm, t.m0 + row) : 0);
+  int coff[4][2];
 #pragma unroll
   for (int j = 0; j < 4; ++j)
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const long long coff = __shfl_sync(0xffffffffu, my_col, j * 8 + fk * 2 + c);
-      if (roff >= 0 && coff >= 0) {
+    for (int c = 0; c < 2; ++c) coff[j][c] = __shfl_sync(0xffffffffu, my_col, j * 8 + zg_ccol(fk, c));
+  if (t.flags & GWSIG_FLAG_ACCUM) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+        if (rok && j * 8 + zg_ccol(fk, c) < ncols) {
+          double2* dst = rowp + coff[j][c];
+          red_add(&dst->x, acc[j][0][c] - acc[j][1][c]);
+          red_add(&dst->y, acc[j][2][c] - acc[j][0][c] - acc[j][1][c]);
+        }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
         const double re = acc[j][0][c] - acc[j][1][c], im = acc[j][2][c] - acc[j][0][c] - acc[j][1][c];
-        double2* dst = cbase + roff + coff;
-        if (accum) { red_add(&dst->x, re); red_add(&dst->y, im); }
-        else *dst = make_double2(re, im);
+        st_pred(rowp + coff[j][c], re, im, rok && j * 8 + zg_ccol(fk, c) < ncols);
       }
-    }
+  }
 }
 
+template <bool kBulk>
 __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p) {
   extern __shared__ double2 zg_smem[];
   double2* As = zg_smem;                              // [kStages3][BK3][LDA3]
@@ -715,7 +745,7 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
   __syncthreads();
 
   if (warp >= kMmaWarps) {
-    loader3(p, As, Bs, full0, empty0, hdr, trec, next_tile, warp - kMmaWarps, lane);
+    loader3<kBulk>(p, As, Bs, full0, empty0, hdr, trec, next_tile, warp - kMmaWarps, lane);
   } else {
     // ================================= MMA WARPS ================================================
     const int fr = lane >> 2, fk = lane & 3;
@@ -741,7 +771,7 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
       }
       if (active) {
         const double2* as = As + stage * BK3 * LDA3 + fk * LDA3 + warp * 8 + fr;
-        const double2* bs = Bs + stage * BK3 * LDB + fk * LDB + fr;
+        const double2* bs = Bs + stage * BK3 * LDB + fk * LDB + zg_bcol(fr);
         const int nk4 = hdr[stage].nk4;
         if (ng == 4) mma3_slot<4>(acc, as, bs, nk4, sa, sb);
         else if (ng == 3) mma3_slot<3>(acc, as, bs, nk4, sa, sb);
@@ -818,11 +848,14 @@ cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t s
     constexpr int smem = kStages3 * BK3 * (LDA3 + LDB) * (int)sizeof(double2);
     if (p.bm != ZG_BM3) return cudaErrorInvalidValue;
     if (!cfg.ok3) {
-      e = cudaFuncSetAttribute(zgemm_grouped_dmma3m, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-      if (e != cudaSuccess) return e;
-      e = cudaFuncSetAttribute(zgemm_grouped_dmma3m, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-      if (e != cudaSuccess) return e;
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cfg.occ3, zgemm_grouped_dmma3m, kThreads3, smem);
+      for (int b = 0; b < 2; ++b) {          // both instantiations: without / with the bulk-copy loader path (option bulk_copies)
+        const void* fn = b ? (const void*)zgemm_grouped_dmma3m<true> : (const void*)zgemm_grouped_dmma3m<false>;
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return e;
+      }
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cfg.occ3, zgemm_grouped_dmma3m<false>, kThreads3, smem);
       if (e != cudaSuccess) return e;
       if (cfg.occ3 < 1) cfg.occ3 = 1;
       cfg.ok3 = true;
@@ -831,7 +864,8 @@ cudaError_t zg_launch(int engine, const ZgParams& p, int num_sms, cudaStream_t s
     long long grid = (long long)num_sms * cfg.occ3;
     if (grid > nchunks) grid = nchunks;
     if (grid < 1) return cudaSuccess;
-    zgemm_grouped_dmma3m<<<(unsigned)grid, kThreads3, smem, stream>>>(p);
+    if (p.use_bulk) zgemm_grouped_dmma3m<true><<<(unsigned)grid, kThreads3, smem, stream>>>(p);
+    else zgemm_grouped_dmma3m<false><<<(unsigned)grid, kThreads3, smem, stream>>>(p);
     return cudaGetLastError();
   }
   // 4M kernel: 4 consumer + 4 producer warps, 128 registers / thread at launch (2 CTAs / SM), redistributed 200 / 56
