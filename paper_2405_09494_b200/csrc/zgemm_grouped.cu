@@ -503,6 +503,17 @@ __device__ __forceinline__ void cp_async16_sz(unsigned smem_dst, const void* gme
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gmem_src), "r"(bytes) : "memory");
 }
 
+// per loader warp: the descriptor of the problem its tile ids are running through and the segment being staged, copied to
+// shared memory ONCE per problem (per segment for multi-segment problems).  Tile ids run through a problem n-tile by n-tile, so
+// what used to be a chain of dependent L2 round trips per tile (bucket table, forward scan, problem, segment) is paid once per
+// problem; per tile the fields come from shared memory.
+struct __align__(16) LoaderCache {
+  gwsig_problem P;     // 144 bytes
+  gwsig_seg S;         // 120 bytes
+  long long pad_;
+};
+static_assert(sizeof(gwsig_problem) == 144 && sizeof(gwsig_seg) == 120, "descriptor layout");
+
 // Loader warp lw OWNS the ring slots whose global index is lw (mod kLoaderWarps3): every loader warp walks the same tile /
 // segment / slot sequence but only fills its own slots, so it has kLoaderWarps3 slot times for one slot's address
 // arithmetic.  Operands move as one 16-byte cp.async per element, lane <-> tile row / column (tile rows lane, lane + 32);
@@ -510,7 +521,7 @@ __device__ __forceinline__ void cp_async16_sz(unsigned smem_dst, const void* gme
 // and W rows in stage 2, V2 rows in stage 3) moves as one bulk copy per k-row instead, issued by lane 0 (UBLKCP).
 template <bool kBulk>
 __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2* Bs, unsigned full0, unsigned empty0, SlotHdr* hdr,
-                                        TileRec* trec, long long* next_tile, int lw, int lane) {
+                                        TileRec* trec, long long* next_tile, LoaderCache& lc, int lw, int lane) {
   const unsigned as0 = (unsigned)__cvta_generic_to_shared(As), bs0 = (unsigned)__cvta_generic_to_shared(Bs);
   const bool leader = lw == 0 && lane == 0;
   int stage = 0, tslot = 0, tbuf = 0;
@@ -518,6 +529,11 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
   int gslot = 0;                  // global slot index modulo kLoaderWarps3
   long long pre = 0;
   if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);
+  long long c_begin = 0, c_end = 0;                                                // tile id range of the cached problem (empty at first)
+  int c_prob = 0, c_tn = 1, c_per = 1;
+  int key_prob = -1, key_batch = -1, key_tm = -1;                                  // what pa[] / sza[] were computed for
+  const double2* pa[2] = {nullptr, nullptr};
+  unsigned sza[2] = {0u, 0u};
   while (true) {
     // tiles are taken kChunk3 consecutive ids at a time: neighbours belong to the same problem (n fastest), so their
     // descriptor loads hit L1 and the chain of dependent L2 round trips is paid once per chunk, not once per tile
@@ -528,37 +544,73 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
     if (chunk0 >= p.total_tiles) break;
     if (leader) pre = (long long)atomicAdd(p.counter, 1ULL);        // lands while this chunk is being staged
     for (long long tile = chunk0; tile < chunk0 + kChunk3 && tile < p.total_tiles; ++tile) {
-      const TileInfo ti = decode_tile(p, tile);
-      const gwsig_problem& P = p.prob[ti.prob];
-      const int M = __ldg(&P.M), N = __ldg(&P.N), flags = __ldg(&P.flags);
+      // consecutive tile ids run through one problem n-tile by n-tile: the problem's fields are decoded when the id leaves the
+      // cached problem's range only (bucket table, forward scan and the descriptor are a chain of dependent loads)
+      if (tile < c_begin || tile >= c_end) {
+        int lo = __ldg(&p.bucket[tile >> ZG_BUCKET_SHIFT]);
+        while (lo + 1 < p.nprob && __ldg(&p.prob[lo + 1].tile_begin) <= tile) ++lo;
+        __syncwarp();                                   // every lane is done with the previous problem's copy
+        if (lane < 18) reinterpret_cast<long long*>(&lc.P)[lane] = __ldg(reinterpret_cast<const long long*>(&p.prob[lo]) + lane);
+        __syncwarp();
+        if (lc.P.seg_count == 1) {
+          if (lane < 15) reinterpret_cast<long long*>(&lc.S)[lane] = __ldg(reinterpret_cast<const long long*>(&p.seg[lc.P.seg_begin]) + lane);
+          __syncwarp();
+        }
+        c_prob = lo;
+        c_tn = lc.P.tiles_n;
+        c_per = lc.P.tiles_m * c_tn;
+        c_begin = lc.P.tile_begin;
+        c_end = c_begin + (long long)lc.P.nbatch * c_per;
+        key_prob = -1;
+      }
+      const gwsig_problem& P = lc.P;
+      TileInfo ti;
+      {
+        const unsigned local = (unsigned)(tile - c_begin);
+        ti.prob = c_prob;
+        ti.batch = (int)(local / (unsigned)c_per);
+        const unsigned r = local - (unsigned)ti.batch * (unsigned)c_per;
+        ti.tm = (int)(r / (unsigned)c_tn);
+        ti.tn = (int)(r - (unsigned)ti.tm * (unsigned)c_tn);
+      }
+      const int M = P.M, N = P.N, flags = P.flags;
       const int m0 = ti.tm * ZG_BM3;
       int n0, ncols;
-      zg_ntile(N, __ldg(&P.tiles_n), ti.tn, n0, ncols);
+      zg_ntile(N, c_tn, ti.tn, n0, ncols);
       const int mrows = min(ZG_BM3, M - m0);
-      const long long a_boff = (long long)ti.batch * __ldg(&P.a_bstride) + (long long)p.t0 * __ldg(&P.a_tstride);
-      const long long b_boff = (long long)ti.batch * __ldg(&P.b_bstride) + (long long)p.t0 * __ldg(&P.b_tstride);
-      const int seg_begin = __ldg(&P.seg_begin), nseg = __ldg(&P.seg_count);
+      const long long a_boff = (long long)ti.batch * P.a_bstride + (long long)p.t0 * P.a_tstride;
+      const long long b_boff = (long long)ti.batch * P.b_bstride + (long long)p.t0 * P.b_tstride;
+      const int seg_begin = P.seg_begin, nseg = P.seg_count;
+      // the A row pointers of a one-segment problem depend on (problem, batch entry, m-tile) only: kept across its n-tiles
+      const bool a_cached = !kBulk && nseg == 1 && c_prob == key_prob && ti.batch == key_batch && ti.tm == key_tm;
       bool first = true;
       for (int s = 0; s < nseg; ++s) {
-        const gwsig_seg& S = p.seg[seg_begin + s];
-        const int K = __ldg(&S.K);
+        if (nseg > 1) {                                 // multi-segment problem (split-K lists): stage this segment's descriptor
+          __syncwarp();
+          if (lane < 15) reinterpret_cast<long long*>(&lc.S)[lane] = __ldg(reinterpret_cast<const long long*>(&p.seg[seg_begin + s]) + lane);
+          __syncwarp();
+        }
+        const gwsig_seg& S = lc.S;
+        const int K = S.K;
         if (K == 0) continue;
         const bool last_seg = s == nseg - 1;
         const int nslots = (K + BK3 - 1) / BK3;
         const int j0 = (lw - gslot + kLoaderWarps3) % kLoaderWarps3;       // this warp's first slot of the segment
         if (j0 < nslots) {
           const bool a_row = kBulk && S.am.div == GWSIG_NODIV && S.am.lo == 1, b_row = kBulk && S.bn.div == GWSIG_NODIV && S.bn.lo == 1;
-          const double2* abase = p.A + __ldg(&S.a_off) + a_boff + (a_row ? m0 : 0);
-          const double2* bbase = p.B + __ldg(&S.b_off) + b_boff + (b_row ? n0 : 0);
+          const double2* abase = p.A + S.a_off + a_boff + (a_row ? m0 : 0);
+          const double2* bbase = p.B + S.b_off + b_boff + (b_row ? n0 : 0);
           // per-lane source pointers of tile rows lane, lane + 32 and tile column lane; lanes outside the tile point at the
           // operand base and copy zero bytes (cp.async zero-fills: no branch in the slot loop, nothing read)
-          const double2* pa[2];
-          unsigned sza[2], szb;
+          unsigned szb;
+          if (!a_cached) {
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const bool v = !a_row && lane + 32 * j < mrows;
-            pa[j] = abase + (v ? idx2(S.am, m0 + lane + 32 * j) : 0);
-            sza[j] = v ? 16u : 0u;
+            for (int j = 0; j < 2; ++j) {
+              const bool v = !a_row && lane + 32 * j < mrows;
+              pa[j] = abase + (v ? idx2(S.am, m0 + lane + 32 * j) : 0);
+              sza[j] = v ? 16u : 0u;
+            }
+            key_prob = nseg == 1 ? c_prob : -1; key_batch = ti.batch; key_tm = ti.tm;
           }
           const bool vb = !b_row && lane < ncols;
           const double2* pb = bbase + (vb ? idx2(S.bn, n0 + lane) : 0);
@@ -582,7 +634,7 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
               if (firstslot) {
                 TileRec& t = trec[tslot];
                 t.mrows = mrows; t.ncols = ncols; t.flags = flags; t.m0 = m0; t.n0 = n0;
-                t.c_off = __ldg(&P.c_off) + (long long)ti.batch * __ldg(&P.c_bstride) + (long long)p.t0 * __ldg(&P.c_tstride);
+                t.c_off = P.c_off + (long long)ti.batch * P.c_bstride + (long long)p.t0 * P.c_tstride;
                 t.cm = P.cm; t.cn = P.cn;
                 h.trec = tslot;
               }
@@ -733,6 +785,7 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
   __shared__ SlotHdr hdr[kStages3];
   __shared__ TileRec trec[kTrec3];
   __shared__ long long next_tile[2];
+  __shared__ LoaderCache lcache[kLoaderWarps3];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned full0 = (unsigned)__cvta_generic_to_shared(&bars[0]);
@@ -745,7 +798,7 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
   __syncthreads();
 
   if (warp >= kMmaWarps) {
-    loader3<kBulk>(p, As, Bs, full0, empty0, hdr, trec, next_tile, warp - kMmaWarps, lane);
+    loader3<kBulk>(p, As, Bs, full0, empty0, hdr, trec, next_tile, lcache[warp - kMmaWarps], warp - kMmaWarps, lane);
   } else {
     // ================================= MMA WARPS ================================================
     const int fr = lane >> 2, fk = lane & 3;
