@@ -341,14 +341,19 @@ void Plan::w_source(int q, int q_first, long long& off, long long& tstride) cons
 static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo; d.div = GWSIG_NODIV; d.pad_ = 0; return d; }
 static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
 
-// the tensor kernels' epilogues keep the element offset of a tile COLUMN (relative to the tile's C base) in 32 bits
-static bool col_offsets_fit(const std::vector<gwsig_problem>& prob) {
+// ranges the tensor kernels rely on: the element offset of a tile COLUMN (relative to the tile's C base) fits 32 bits, and
+// every index that goes through a two-level map (rows, columns, k) is below 2^22 (the kernels divide with a float reciprocal)
+static bool kernel_ranges_ok(const std::vector<gwsig_problem>& prob, const std::vector<gwsig_seg>& seg) {
+  const long long lim = 1LL << 22;
   for (const auto& P : prob) {
     if (P.N <= 0) continue;
+    if (P.M >= lim || P.N >= lim) return false;
     const long long n = P.N - 1;
     const long long off = P.cn.div == GWSIG_NODIV ? n * P.cn.lo : (n / P.cn.div) * P.cn.hi + std::min<long long>(P.cn.div - 1, n) * P.cn.lo;
     if (off < 0 || off >= (1LL << 31)) return false;
   }
+  for (const auto& S : seg)
+    if (S.K >= lim) return false;
   return true;
 }
 
@@ -597,7 +602,7 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
     sorted[i] = P;
   }
   out.prob.swap(sorted);
-  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
+  if (!kernel_ranges_ok(out.prob, out.seg)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   {
@@ -736,7 +741,7 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
   }
-  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
+  if (!kernel_ranges_ok(out.prob, out.seg)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -820,7 +825,7 @@ int Plan::build_vtransform(long long p0, long long np, int step, StagePlan& out)
     P.tile_begin = tb;
     tb += (long long)P.nbatch * P.tiles_m * P.tiles_n;
   }
-  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
+  if (!kernel_ranges_ok(out.prob, out.seg)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -853,7 +858,7 @@ int Plan::build_gridtransform(int nq, int nin, int nout, StagePlan& out) const {
     tb += (long long)P.tiles_m * P.tiles_n;
     out.seg.push_back(S); out.prob.push_back(P);
   }
-  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
+  if (!kernel_ranges_ok(out.prob, out.seg)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
@@ -957,7 +962,7 @@ int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePla
     sorted[i] = P;
   }
   out.prob.swap(sorted);
-  if (!col_offsets_fit(out.prob)) return GWSIG_ERR_ARG;
+  if (!kernel_ranges_ok(out.prob, out.seg)) return GWSIG_ERR_ARG;
   out.ntiles = tb;
   out.bucket.assign((size_t)((tb + (1 << ZG_BUCKET_SHIFT) - 1) >> ZG_BUCKET_SHIFT) + 1, 0);
   size_t pi = 0;
