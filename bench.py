@@ -492,6 +492,12 @@ def reference_main(args, rank, world):
     print(json.dumps(line))
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
+# capture of this command (profiles/r2_ncu_default_engine_cfg3.md); ncu never runs inside bench.py, so every other
+# (workload, mode, engine) reports null.  Key: (workload, mode, engine option, stage index 0..2).
+NCU_DRAM_BYTES_PER_LAUNCH = {("cfg3", "ibz_block", 0, 1): 7.82e9}
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -610,7 +616,10 @@ def main():
     dom = int(np.argmax([t1, t2, t3]))
     ach = sf[dom] / max((t1, t2, t3)[dom], 1e-12) / 1e12
     line["roofline"] = {"bound": "tensor", "kernel": ("stage1_X=VG", "stage2_Y=WX", "stage3_S+=YV")[dom] + (" (zgemm_grouped_dmma3m)" if (args.engine == 3 or (args.engine == 0 and dom in (0, 1))) else " (zgemm_grouped_dmma)"),
-                        "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                        "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, args.mode, args.engine, dom)),
+                        "traffic_note": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r2_ncu_default_engine_cfg3.md): "
+                                        "X is read from and Y written to HBM; null where no ncu capture of this command is committed",
                         "peak_measured_dmma_probe": probe_tf,
                         "peak_source": "FP64 tensor (DMMA) peak derived from unit counts x max clock, 148 x 128 flop/clk x 1.965 GHz "
                                        "(MEASURED_PEAKS.json has no FP64 entry); peak_measured_dmma_probe is the register-only DMMA issue-rate "
