@@ -342,18 +342,22 @@ static inline gwsig_idx2 lvl1(long long lo) { gwsig_idx2 d; d.hi = 0; d.lo = lo;
 static inline gwsig_idx2 lvl2(int div, long long hi, long long lo) { gwsig_idx2 d; d.hi = hi; d.lo = lo; d.div = div; d.pad_ = 0; return d; }
 
 // ranges the tensor kernels rely on: the element offset of a tile COLUMN (relative to the tile's C base) fits 32 bits, and
-// every index that goes through a two-level map (rows, columns, k) is below 2^22 (the kernels divide with a float reciprocal)
+// every index that goes through a TWO-LEVEL map (rows, columns, k) is below 2^22 (the kernels divide with a float reciprocal);
+// single-level maps carry no such limit
 static bool kernel_ranges_ok(const std::vector<gwsig_problem>& prob, const std::vector<gwsig_seg>& seg) {
   const long long lim = 1LL << 22;
+  auto two = [](const gwsig_idx2& d) { return d.div != GWSIG_NODIV; };
   for (const auto& P : prob) {
     if (P.N <= 0) continue;
-    if (P.M >= lim || P.N >= lim) return false;
+    if ((two(P.cm) && P.M >= lim) || (two(P.cn) && P.N >= lim)) return false;
+    for (int s = P.seg_begin; s < P.seg_begin + P.seg_count; ++s) {
+      const gwsig_seg& S = seg[s];
+      if ((two(S.am) && P.M >= lim) || (two(S.bn) && P.N >= lim) || ((two(S.ak) || two(S.bk)) && S.K >= lim)) return false;
+    }
     const long long n = P.N - 1;
     const long long off = P.cn.div == GWSIG_NODIV ? n * P.cn.lo : (n / P.cn.div) * P.cn.hi + std::min<long long>(P.cn.div - 1, n) * P.cn.lo;
     if (off < 0 || off >= (1LL << 31)) return false;
   }
-  for (const auto& S : seg)
-    if (S.K >= lim) return false;
   return true;
 }
 
