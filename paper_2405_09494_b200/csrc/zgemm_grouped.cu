@@ -1,11 +1,11 @@
 // Grouped / ragged batched complex-FP64 GEMM on the FP64 tensor pipe (sm_100a).
 //
-// TWO tensor-core kernels share the loader, the tile scheduler and the descriptors:
-//   zgemm_grouped_dmma3m (engine 0, default): Karatsuba / "3M" complex product -- three REAL products
-//       P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi),  re = P1 - P2,  im = P3 - P1 - P2  (25 % fewer DMMA than 4M);
-//       16 MMA warps, one row group of the tile each, fed by ONE loader warp with bulk async copies (UBLKCP);
-//       details above the kernel
-//   zgemm_grouped_dmma   (engine 2): the conventional four-product kernel (engine v3 of round 1), described below.
+// TWO tensor-core kernels share the tile scheduler and the descriptors:
+//   zgemm_grouped_dmma3m (engine 3; the default engine runs stages 1 and 2 on it): Karatsuba / "3M" complex product -- three
+//       REAL products P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi),  re = P1 - P2,  im = P3 - P1 - P2  (25 % fewer DMMA than 4M);
+//       two CTAs per SM of 8 MMA warps (one 8-row group of a 64-row tile each) + 2 loader warps; details above the kernel
+//   zgemm_grouped_dmma   (engine 2; the default engine runs stage 3 and the Eq. 28 unfold on it): the conventional
+//       four-product kernel (engine v3 of round 1), described below.
 //
 // Serves the three contraction stages of the GW self-energy (Algorithm 4 lines 5, 7, 8 of
 // arXiv 2405.09494).  Descriptors: include/gwsig_plan.h.  Design: DESIGN.md section 5.
