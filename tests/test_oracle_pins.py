@@ -393,3 +393,83 @@ def test_dyson_p_loops_scalar_series_resolvent():
         w = Tf @ d[0, :, j]
         assert np.abs(Pd[0, :, j, j] - Tb @ (w / (1 - w))).max() < 1e-13
     assert np.abs(Pd[..., 0, 1]).max() == 0
+
+
+# ---- Hartree J, Eq. 21b ----------------------------------------------------------------
+def test_hartree_brute_vs_ref_scalar_and_einsum():
+    from oracle.hartree_oracle import aux_density, hartree_brute, hartree_ref
+    rng = np.random.default_rng(12)
+    nk, nao, naux = 3, 2, 3
+    gamma = rng.standard_normal((nk, nao, nao)) + 1j * rng.standard_normal((nk, nao, nao))            # no structure assumed
+    V = rng.standard_normal((nk, naux, nao, nao)) + 1j * rng.standard_normal((nk, naux, nao, nao))
+    ks = [0, 2]
+    brute = hartree_brute(nk, gamma, lambda k: V[k], ks)
+    ref = hartree_ref(nk, lambda k: gamma[k], lambda k: V[k], ks)
+    assert np.abs(brute - ref).max() < 1e-13 * np.abs(brute).max()
+    # an independent statement of Eq. 21b: the index pattern typed out once more, as one einsum
+    ein = np.einsum("kQij,pab,pQba->kij", V[ks], gamma, V) / nk
+    assert np.abs(ein - ref).max() < 1e-13 * np.abs(ref).max()
+    # a transposed gamma / V (gamma_ab V_ab instead of gamma_ab V_ba) is a different number
+    wrong = np.einsum("kQij,pab,pQab->kij", V[ks], gamma, V) / nk
+    assert np.abs(wrong - ref).max() > 1e-2 * np.abs(ref).max()
+    # scalar closed form: nao = naux = 1  ->  J^k = v_k (1/Nk) sum_k' gamma_k' v_k'
+    g1 = rng.standard_normal((nk, 1, 1)) + 1j * rng.standard_normal((nk, 1, 1))
+    v1 = rng.standard_normal((nk, 1, 1, 1)) + 1j * rng.standard_normal((nk, 1, 1, 1))
+    J1 = hartree_ref(nk, lambda k: g1[k], lambda k: v1[k], range(nk))
+    want = v1[:, 0, 0, 0] * (g1[:, 0, 0] * v1[:, 0, 0, 0]).sum() / nk
+    assert np.abs(J1[:, 0, 0] - want).max() < 1e-14 * np.abs(want).max()
+    # Hartree energy identity: (1/Nk) sum_k tr[gamma^k J^k] = sum_Q rho_Q^2
+    rho = aux_density(nk, lambda k: gamma[k], lambda k: V[k])
+    Jall = hartree_ref(nk, lambda k: gamma[k], lambda k: V[k], range(nk))
+    e = sum(np.trace(gamma[k] @ Jall[k]) for k in range(nk)) / nk
+    assert abs(e - (rho * rho).sum()) < 1e-13 * abs(e)
+
+
+def test_hartree_invariances():
+    from oracle.hartree_oracle import hartree_ref
+    rng = np.random.default_rng(13)
+    nk, nao, naux = 4, 3, 5
+    gamma = rng.standard_normal((nk, nao, nao)) + 1j * rng.standard_normal((nk, nao, nao))
+    V = rng.standard_normal((nk, naux, nao, nao)) + 1j * rng.standard_normal((nk, naux, nao, nao))
+    J = hartree_ref(nk, lambda k: gamma[k], lambda k: V[k], range(nk))
+    # orbital unitaries T_k (independent per k): gamma -> T gamma T^dagger, V_Q -> T V_Q T^dagger  =>  rho unchanged, J -> T J T^dagger
+    T = [np.linalg.qr(rng.standard_normal((nao, nao)) + 1j * rng.standard_normal((nao, nao)))[0] for _ in range(nk)]
+    J2 = hartree_ref(nk, lambda k: T[k] @ gamma[k] @ T[k].conj().T, lambda k: np.einsum("ip,Qpq,jq->Qij", T[k], V[k], T[k].conj()), range(nk))
+    for k in range(nk):
+        assert np.abs(J2[k] - T[k] @ J[k] @ T[k].conj().T).max() < 1e-13 * np.abs(J).max()
+    # a real orthogonal rotation of the auxiliary index (both V carry Q un-conjugated at q = 0) leaves J unchanged ...
+    S = np.linalg.qr(rng.standard_normal((naux, naux)))[0]
+    J3 = hartree_ref(nk, lambda k: gamma[k], lambda k: np.einsum("PQ,Qij->Pij", S, V[k]), range(nk))
+    assert np.abs(J3 - J).max() < 1e-13 * np.abs(J).max()
+    # ... a complex unitary one does not
+    Sc = np.linalg.qr(rng.standard_normal((naux, naux)) + 1j * rng.standard_normal((naux, naux)))[0]
+    J4 = hartree_ref(nk, lambda k: gamma[k], lambda k: np.einsum("PQ,Qij->Pij", Sc, V[k]), range(nk))
+    assert np.abs(J4 - J).max() > 1e-3 * np.abs(J).max()
+    # linear in gamma
+    g2 = rng.standard_normal((nk, nao, nao)) + 1j * rng.standard_normal((nk, nao, nao))
+    Jb = hartree_ref(nk, lambda k: g2[k], lambda k: V[k], range(nk))
+    Jab = hartree_ref(nk, lambda k: gamma[k] + 2.0 * g2[k], lambda k: V[k], range(nk))
+    assert np.abs(Jab - J - 2.0 * Jb).max() < 1e-13 * np.abs(Jab).max()
+
+
+@pytest.mark.parametrize("name", ["toy_diamond", "toy_wurtzite"])
+def test_hartree_on_a_symmetric_crystal(name):
+    """Hermitian gamma and the generator's V^{kk}(Q)_{ij} = conj(V^{kk}(Q)_{ji}): rho is real and J Hermitian; J transforms like
+    every one-body matrix, J(g k) = O J(k) O^dagger (Eq. 22)."""
+    from oracle.hartree_oracle import aux_density, hartree_ref
+    inp = make_inputs(name)
+    cr, sg, km = inp.cr, inp.cr.sg, inp.cr.kmesh
+    G = np.stack([inp.G_k(k) for k in range(inp.nk)])
+    gamma = -G[:, -1]                                           # gamma^k = G^k(0^-) = -G^k(beta)
+    Vd = inp.V_pairs(range(inp.nk), range(inp.nk))              # V^{kk}
+    rho = aux_density(inp.nk, lambda k: gamma[k], lambda k: Vd[k])
+    assert np.abs(rho.imag).max() < 1e-12 * np.abs(rho).max() and np.abs(rho).max() > 1e-6
+    J = hartree_ref(inp.nk, lambda k: gamma[k], lambda k: Vd[k], range(inp.nk))
+    scale = np.abs(J).max()
+    assert np.abs(J - J.conj().transpose(0, 2, 1)).max() < 1e-12 * scale
+    _, _, _, rot = km.stars(sg)
+    for g in range(sg.nops):
+        for k in range(km.nk):
+            kt = rot[g, k]
+            O = rep_at_k(cr.P_ao[g], cr.ao_atom, sg.shift[g], km.frac[kt])
+            assert np.abs(J[kt] - O @ J[k] @ O.conj().T).max() < 1e-11 * scale
