@@ -66,7 +66,8 @@ enum {
   GWSIG_KIND_VTRANSFORM = 6, /* Eq. 27 block transform of V (gwsig_block_transform_v) */
   GWSIG_KIND_GRIDXFORM = 7,  /* tau <-> i Omega transforms of gwsig_dyson_p                  */
   GWSIG_KIND_DYSON = 8,      /* batched [1 - P0]^{-1} P0 solve of gwsig_dyson_p             */
-  GWSIG_NKINDS = 9
+  GWSIG_KIND_HARTREE = 9,    /* the two kernels of gwsig_hartree_eval (Eq. 21b)             */
+  GWSIG_NKINDS = 10
 };
 
 /* ---- life cycle ------------------------------------------------------------------------ */
@@ -177,6 +178,17 @@ int gwsig_sigma_eval_host(gwsig_ctx* ctx, const void* hG, const void* hV_all, co
  * sigma_abort) exactly as sigma_begin is; exchange_eval = begin + one push of all pairs + end.                       */
 int gwsig_exchange_begin(gwsig_ctx* ctx, const void* dGamma, void* dK, void* stream);
 int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, void* dK, void* stream);
+
+/* ---- N2 (second half): the Hartree self-energy J^k -------------------------------------------
+ * J^k_ij = (1/Nk) sum_{k'} sum_{ab} sum_Q V^{kk}_{ij}(Q) gamma^{k'}_{ab} V^{k'k'}_{ba}(Q)      (Eq. 21b), one spin channel
+ * (the sum over sigma_1 is a factor the caller applies), gamma^k = G^k(tau = 0^-).  Two HBM-bound kernels: the
+ * auxiliary density rho_Q = (1/Nk) sum_{k'} tr[gamma^{k'} V^{k'k'}(Q)] (one CTA per Q, fixed summation order: bit-reproducible), then
+ * J^k = sum_Q V^{kk}(Q) rho_Q.  Orbital basis, ALL Nk points of the mesh in the order of the k index, whatever the context's mode
+ * (only set_lattice is needed; no symmetry is used):
+ *   dGamma (dev, in) [Nk][nao][nao]      dVdiag (dev, in) [Nk][naux][nao][nao] = V^{kk}_{Q,ij}      dJ (dev, out) [Nk][nao][nao]
+ * complex128, caller-owned.  Asynchronous on `stream`.  Errors: GWSIG_ERR_ARG (NULL pointer, no lattice), GWSIG_ERR_ORDER
+ * (an evaluation is open), GWSIG_ERR_CUDA.                                                                                  */
+int gwsig_hartree_eval(gwsig_ctx* ctx, const void* dGamma, const void* dVdiag, void* dJ, void* stream);
 
 /* ---- N3: the auxiliary function P from the bare bubble ------------------------------------
  * P^q(i Omega_n) = [1 - P0^q(i Omega_n)]^{-1} P0^q(i Omega_n)  (Eq. 19a),  P^q(tau) by the inverse transform

@@ -76,6 +76,7 @@ struct gwsig_ctx {
   DevBuf gbz, wring, xbuf, ybuf, sigacc, counters, epidesc, probe_sink;
   DevBuf oblk_ao, oblk_aux, unf_tmp, partial;
   DevBuf dys_flag;                               // N3: singular-matrix flag of the Eq. 19 solve
+  DevBuf hart_rho;                               // N2: auxiliary density rho_Q of the Hartree term (Eq. 21b)
   DevBuf u_ao_dev, u_aux_dev;                    // N4: the adapted bases on the device (set_blocks with U)
   DevBuf grev, p0acc, p0desc;                    // N1 (Eq. 20): G(beta - tau) on the full zone, the P0 accumulator, its epilogue descriptors
   bool in_p0 = false;
@@ -381,7 +382,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->dys_flag, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->dys_flag, &ctx->hart_rho, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -774,6 +775,27 @@ int gwsig_exchange_eval(gwsig_ctx* ctx, const void* dGamma, const void* dV_all, 
   rc = gwsig_sigma_push_pairs(ctx, 0, ctx->plan.npairs, dV_all);
   if (rc) { ctx->in_eval = false; ctx->exchange = false; return rc; }
   return gwsig_sigma_end(ctx);
+}
+
+/* ---- N2: Hartree J, Eq. 21b ---------------------------------------------------------------------------------- */
+int gwsig_hartree_eval(gwsig_ctx* ctx, const void* dGamma, const void* dVdiag, void* dJ, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (!P.have_lattice) return fail(ctx, GWSIG_ERR_ARG, "hartree_eval: call set_lattice first");
+  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "hartree_eval: an evaluation is open");
+  if (!dGamma || !dVdiag || !dJ) return fail(ctx, GWSIG_ERR_ARG, "hartree_eval: NULL device pointer");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)stream;
+  ctx->ev_used.clear();
+  ctx->launches = 0;
+  CU(ctx->hart_rho.ensure((size_t)P.naux * sizeof(double2)));
+  if ((rc = tic(ctx, GWSIG_KIND_HARTREE))) return rc;
+  CU(launch_hartree((const double2*)dGamma, (const double2*)dVdiag, (double2*)ctx->hart_rho.p, (double2*)dJ, P.nk, P.nao, P.naux, ctx->stream));
+  if ((rc = toc(ctx))) return rc;
+  ctx->launches += 2;
+  return GWSIG_OK;
 }
 
 /* ---- N3: P^q(tau) from the bare bubble, Eq. 19 ------------------------------------------------------- */

@@ -244,6 +244,59 @@ cudaError_t launch_dyson_solve(double2* X, int nmat, int n, double2* work, int n
   return cudaGetLastError();
 }
 
+// Eq. 21b, first factor: rho_Q = scale * sum_k sum_{ab} gamma^k[a][b] V^{kk}[Q][b][a], one CTA per Q.  The thread
+// index runs over (k, b, a) with a fastest, so V is read in contiguous runs; every thread sums its terms in a fixed order and the
+// block reduction is a fixed tree: the result is bit-reproducible.  HBM-bound: V^{kk} is read once (nk naux nao^2 16 bytes).
+__global__ void __launch_bounds__(256) hartree_rho_kernel(const double2* __restrict__ gamma, const double2* __restrict__ Vd, double2* rho,
+                                                          int nk, int nao, int naux, double scale) {
+  __shared__ double red_r[256], red_i[256];
+  const int Q = blockIdx.x, tid = threadIdx.x, n2 = nao * nao;
+  double sr = 0.0, si = 0.0;
+  for (long long e = tid; e < (long long)nk * n2; e += blockDim.x) {
+    const int k = (int)(e / n2), ba = (int)(e - (long long)k * n2);
+    const int b = ba / nao, a = ba - b * nao;
+    const double2 v = Vd[((long long)k * naux + Q) * n2 + ba];          // V^{kk}[Q][b][a]
+    const double2 g = gamma[(long long)k * n2 + a * nao + b];           // gamma^k[a][b]
+    sr += g.x * v.x - g.y * v.y;
+    si += g.x * v.y + g.y * v.x;
+  }
+  red_r[tid] = sr; red_i[tid] = si;
+  __syncthreads();
+  for (int s_ = blockDim.x / 2; s_ > 0; s_ >>= 1) {
+    if (tid < s_) { red_r[tid] += red_r[tid + s_]; red_i[tid] += red_i[tid + s_]; }
+    __syncthreads();
+  }
+  if (tid == 0) rho[Q] = make_double2(scale * red_r[0], scale * red_i[0]);
+}
+
+// Eq. 21b, second factor: J^k[i][j] = sum_Q V^{kk}[Q][i][j] rho_Q, one thread per (k, i, j), Q ascending.  HBM-bound: the second
+// read of V^{kk}.
+__global__ void __launch_bounds__(256) hartree_j_kernel(const double2* __restrict__ Vd, const double2* __restrict__ rho, double2* J, int nk,
+                                                        int nao, int naux) {
+  const int n2 = nao * nao;
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (long long)nk * n2) return;
+  const int k = (int)(e / n2), ij = (int)(e - (long long)k * n2);
+  const double2* v = Vd + (long long)k * naux * n2 + ij;
+  double sr = 0.0, si = 0.0;
+  for (int Q = 0; Q < naux; ++Q) {
+    const double2 x = v[(long long)Q * n2], r = rho[Q];
+    sr += x.x * r.x - x.y * r.y;
+    si += x.x * r.y + x.y * r.x;
+  }
+  J[e] = make_double2(sr, si);
+}
+
+cudaError_t launch_hartree(const double2* gamma, const double2* Vd, double2* rho, double2* J, int nk, int nao, int naux, cudaStream_t stream) {
+  if (nk <= 0 || nao <= 0 || naux <= 0) return cudaSuccess;
+  hartree_rho_kernel<<<(unsigned)naux, 256, 0, stream>>>(gamma, Vd, rho, nk, nao, naux, 1.0 / (double)nk);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const long long tot = (long long)nk * nao * nao;
+  hartree_j_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(Vd, rho, J, nk, nao, naux);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream) {
   if (ngroups <= 0) return cudaSuccess;
   for (int g0 = 0; g0 < ngroups; g0 += 65535) {

@@ -36,6 +36,7 @@ struct RedGroupDev {      // = gwsig::RedGroup (plan.hpp)
 // acc[block] += sum over the block's partial tiles IN PART ORDER (deterministic stage 3)
 cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream);
 // Eq. 19a per matrix: X <- [1 - X]^{-1} X in place, nmat matrices [n][n] back to back; work = per-CTA scratch [ncta][n][2n]
+cudaError_t launch_hartree(const double2* gamma, const double2* Vd, double2* rho, double2* J, int nk, int nao, int naux, cudaStream_t stream);
 cudaError_t launch_dyson_solve(double2* X, int nmat, int n, double2* work, int ncta, int* fail_flag, cudaStream_t stream);
 // dst[k][n] = src[k][ntau-1-n] for nk matrices-over-tau of `elems` complex numbers each (G(beta - tau) for Eq. 20)
 cudaError_t launch_reverse_tau(const double2* src, double2* dst, int nk, int ntau, long long elems, cudaStream_t stream);

@@ -429,6 +429,35 @@ def test_cfg5_sampled():
     _sampled("cfg5", 1, lambda wedge: [wedge[0]], [135], pushes_q=64)
 
 
+@pytest.mark.parametrize("name", ["cfg1", "toy_diamond4", "toy_wurtzite", "cfg2"])
+def test_hartree_eq21b(name):
+    """J^k (Eq. 21b) through gwsig_hartree_eval against oracle/hartree_oracle.py at every mesh point; twice on the
+    same inputs: the summation order is fixed, the results are bit-identical."""
+    B = _B()
+    torch = _torch()
+    from oracle.hartree_oracle import hartree_ref
+    from paper_2405_09494_b200.pack import Configured
+    inp = get_inputs(name)
+    lib = B.Gwsig(device=0)
+    mesh = inp.kmesh.N
+    Configured(lib, 0, np.eye(3), mesh, inp.nao, inp.naux, inp.ntau, inp.beta, None, None, None)
+    nk = inp.nk
+    G = np.stack([inp.G_k(k) for k in range(nk)]) if hasattr(inp, "G_k") else inp.G_full()
+    gamma = np.ascontiguousarray(-G[:, -1])                          # gamma^k = G^k(0^-) = -G^k(beta)  (PAPER.md:194)
+    Vd = np.ascontiguousarray(inp.V_pairs(range(nk), range(nk)))     # V^{kk}_{Q,ij}
+    ref = hartree_ref(nk, lambda k: gamma[k], lambda k: Vd[k], range(nk))
+    dG, dV = torch.from_numpy(gamma).cuda(), torch.from_numpy(Vd).cuda()
+    outs = []
+    for _ in range(2):
+        dJ = torch.full((nk * inp.nao * inp.nao,), float("nan"), dtype=torch.complex128, device="cuda")
+        lib.hartree_eval(dG, dV, dJ, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        outs.append(dJ.cpu().numpy().reshape(nk, inp.nao, inp.nao))
+    worst = max(rel_err(outs[0][k], ref[k]) for k in range(nk))
+    assert worst <= TOL, worst
+    assert np.array_equal(outs[0], outs[1])
+
+
 def test_hermitize_option_and_observed_hermiticity():
     B, inp, cfg, G, W, V = _setup("toy_diamond", 1)
     s0 = run_gpu(cfg, G, W, V)
