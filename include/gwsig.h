@@ -233,6 +233,18 @@ int gwsig_dyson_solve_noalloc(const void* dA, void* dX, int nmat, int n, void* d
  * the CPU before the calculation.  Synchronises the stream.                                              */
 int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, void* dV_packed, void* stream);
 
+/* ---- N4, second half: allowed-block detection on the device ("only non-zero blocks are considered") ----
+ * For pairs p0 .. p0+np-1 the Eq. 27 transform of the orbital-basis tensors is carried out for EVERY block (three grouped-GEMM
+ * launches per sub-batch, the last one dense) and the largest |.| of each candidate block (p, alpha, iota) is reduced on the
+ * device.  Needs GWSIG_IBZ_BLOCK and set_blocks WITH the bases U_ao, U_aux; needs NO triples: this is the call whose result the
+ * caller thresholds (e.g. 1e-9 of max |V|; forbidden blocks come out below 1e-13 of it) to build the lists for gwsig_set_triples.
+ *   dV_dense (dev, in)  [np][naux][nao][nao] = V^{k2,k1}_{Q,bj} back to back in pair order (as for gwsig_block_transform_v)
+ *   d_maxabs (dev, out) double [np][mb_aux][mb_ao][mb_ao]: entry ((pair * mb_aux + p) * mb_ao + alpha) * mb_ao + iota, zero for block
+ *                       indices a mesh point does not have; mb_aux / mb_ao >= the largest number of auxiliary / orbital blocks of
+ *                       any mesh point, mb_aux * mb_ao^2 <= 6144.
+ * Synchronises the stream.  Errors: GWSIG_ERR_ARG, GWSIG_ERR_ORDER, GWSIG_ERR_CUDA.                                        */
+int gwsig_block_maxabs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, int mb_aux, int mb_ao, void* d_maxabs, void* stream);
+
 /* ---- N1: bare bubble ---------------------------------------------------------------
  * P0^q_{QQ'}(tau) = -(1/Nk) sum_k sum_{abcd} V^{k,k+q}_{Q,da} G^k_{cd}(-tau) G^{k+q}_{ab}(tau) V^{k+q,k}_{Q',bc}   (Eq. 20,
  * PAPER.md:179-184; one spin channel) in the order of Algorithm 3: X1 = V G^k(-tau), X2 = V G^{k+q}(tau),

@@ -37,7 +37,7 @@ EXPORTS = ["gwsig_create", "gwsig_destroy", "gwsig_last_error", "gwsig_set_latti
            "gwsig_plan_get", "gwsig_probe_fp64", "gwsig_kernel_times", "gwsig_sigma_abort", "gwsig_sigma_eval_host",
            "gwsig_set_output_points", "gwsig_exchange_begin", "gwsig_exchange_eval",
            "gwsig_p0_begin", "gwsig_p0_push_pairs", "gwsig_p0_end", "gwsig_p0_eval", "gwsig_block_transform_v", "gwsig_dyson_p",
-           "gwsig_dyson_solve_noalloc", "gwsig_hartree_eval"]
+           "gwsig_dyson_solve_noalloc", "gwsig_hartree_eval", "gwsig_block_maxabs"]
 
 _vp, _i, _i64, _d = C.c_void_p, C.c_int, C.c_int64, C.c_double
 _sig = {
@@ -59,6 +59,7 @@ _sig = {
     "gwsig_dyson_p": [_vp, _vp, _vp, _vp, _i, _vp, _vp],
     "gwsig_dyson_solve_noalloc": [_vp, _vp, _i, _i, _vp, _vp, C.c_char_p, _i],
     "gwsig_hartree_eval": [_vp, _vp, _vp, _vp, _vp],
+    "gwsig_block_maxabs": [_vp, _i64, _i64, _vp, _i, _i, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(_lib, _name).argtypes = _args
@@ -239,6 +240,9 @@ class Gwsig:
 
     def block_transform_v(self, p0, np_, dV_dense, dV_packed, stream=0):
         self._ck(_lib.gwsig_block_transform_v(self._h, p0, np_, _ptr(dV_dense), _ptr(dV_packed), stream or None))
+
+    def block_maxabs(self, p0, np_, dV_dense, mb_aux, mb_ao, d_maxabs, stream=0):
+        self._ck(_lib.gwsig_block_maxabs(self._h, int(p0), int(np_), _ptr(dV_dense), int(mb_aux), int(mb_ao), _ptr(d_maxabs), stream or None))
 
     def hartree_eval(self, dGamma, dVdiag, dJ, stream=0):
         self._ck(_lib.gwsig_hartree_eval(self._h, _ptr(dGamma), _ptr(dVdiag), _ptr(dJ), stream or None))

@@ -907,6 +907,94 @@ int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* 
   return GWSIG_OK;
 }
 
+/* ---- N4: allowed-block detection on the device (Eq. 27) ------------------------------------------------------ */
+int gwsig_block_maxabs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, int mb_aux, int mb_ao, void* d_maxabs, void* stream) {
+  if (!ctx) return GWSIG_ERR_ARG;
+  Plan& P = ctx->plan;
+  if (P.mode != GWSIG_IBZ_BLOCK || !P.have_blocks) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: needs GWSIG_IBZ_BLOCK with set_blocks");
+  if (!P.have_U) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: set_blocks must be given the adapted bases U_ao, U_aux");
+  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "block_maxabs: an evaluation is open");
+  if (np < 1 || p0 < 0 || p0 + np > P.npairs) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: bad pair range");
+  if (!dV_dense || !d_maxabs) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: NULL device pointer");
+  int nb_aux = 0, nb_ao = 0;
+  for (int k = 0; k < P.nk; ++k) {
+    nb_aux = std::max(nb_aux, (int)P.aux_off[k].size() - 1);
+    nb_ao = std::max(nb_ao, (int)P.ao_off[k].size() - 1);
+  }
+  if (mb_aux < nb_aux || mb_ao < nb_ao) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: mb_aux / mb_ao smaller than the largest block count of a mesh point");
+  const long long ncand = (long long)mb_aux * mb_ao * mb_ao;
+  if (ncand * 8 > 48 * 1024) return fail(ctx, GWSIG_ERR_ARG, "block_maxabs: more than 6144 candidate blocks per pair");
+  int rc = ensure_cuda(ctx);
+  if (rc) return rc;
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)stream;
+  if ((rc = prepare_tables(ctx))) return rc;
+  CU(ctx->counters.ensure(gwsig_ctx::kCounterSlots * sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(ctx->counters.p, 0, gwsig_ctx::kCounterSlots * sizeof(unsigned long long), ctx->stream));
+  ctx->counter_slot = 0;
+  ctx->ev_used.clear();
+  ctx->launches = 0;
+  // block label of every basis function at every mesh point
+  std::vector<int> lab_aux((size_t)P.nk * P.naux), lab_ao((size_t)P.nk * P.nao);
+  for (int k = 0; k < P.nk; ++k) {
+    for (size_t b = 0; b + 1 < P.aux_off[k].size(); ++b)
+      for (int i = P.aux_off[k][b]; i < P.aux_off[k][b + 1]; ++i) lab_aux[(size_t)k * P.naux + i] = (int)b;
+    for (size_t b = 0; b + 1 < P.ao_off[k].size(); ++b)
+      for (int i = P.ao_off[k][b]; i < P.ao_off[k][b + 1]; ++i) lab_ao[(size_t)k * P.nao + i] = (int)b;
+  }
+  DevBuf d_lab_aux, d_lab_ao, d_qkk;
+  auto cleanup = [&]() { d_lab_aux.release(); d_lab_ao.release(); d_qkk.release(); };
+  if ((rc = upload(ctx, d_lab_aux, lab_aux)) || (rc = upload(ctx, d_lab_ao, lab_ao))) { cleanup(); return rc; }
+  cudaError_t e = cudaMemsetAsync(d_maxabs, 0, (size_t)np * ncand * sizeof(double), ctx->stream);
+  if (e != cudaSuccess) { cleanup(); return cuda_fail(ctx, e, "block_maxabs memset"); }
+  const long long xs = (long long)P.naux * P.nao * P.nao;
+  size_t free_b = 0, total_b = 0;
+  e = cudaMemGetInfo(&free_b, &total_b);
+  if (e != cudaSuccess) { cleanup(); return cuda_fail(ctx, e, "cudaMemGetInfo"); }
+  const double avail = 0.4 * ((double)free_b + (double)ctx->xbuf.bytes + (double)ctx->ybuf.bytes);
+  const double budget = std::min((double)ctx->scratch_mib * 1048576.0, std::max(avail, 64.0 * 1048576.0)) / (2.0 * sizeof(double2));
+  const long long ns_max = std::max<long long>(1, (long long)(budget / (double)xs));
+  for (long long s0 = p0; s0 < p0 + np; s0 += ns_max) {
+    const long long ns = std::min<long long>(ns_max, p0 + np - s0);
+    if ((e = ctx->xbuf.ensure((size_t)xs * ns * sizeof(double2))) != cudaSuccess || (e = ctx->ybuf.ensure((size_t)xs * ns * sizeof(double2))) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(ctx, e, "block_maxabs scratch");
+    }
+    const double2* Vsub = (const double2*)dV_dense + (s0 - p0) * xs;
+    const int steps[3] = {1, 2, 4};                  // T1 -> xbuf, T2 -> ybuf, T3 (dense, every block) -> xbuf
+    for (int si = 0; si < 3; ++si) {
+      StagePlan sp;
+      rc = P.build_vtransform(s0, ns, steps[si], sp);
+      if (rc) { cleanup(); return fail(ctx, rc, "internal: build_vtransform failed"); }
+      DevStage d;
+      d.nprob = (int)sp.prob.size(); d.ntiles = sp.ntiles;
+      if ((rc = upload(ctx, d.prob, sp.prob)) || (rc = upload(ctx, d.seg, sp.seg)) || (rc = upload(ctx, d.bucket, sp.bucket))) { cleanup(); return rc; }
+      const double2* A = si == 0 ? Vsub : si == 1 ? (const double2*)ctx->xbuf.p : (const double2*)ctx->ybuf.p;
+      const double2* Bm = (const double2*)(si == 0 ? ctx->u_aux_dev.p : ctx->u_ao_dev.p);
+      double2* C = si == 1 ? (double2*)ctx->ybuf.p : (double2*)ctx->xbuf.p;
+      rc = run_stage(ctx, GWSIG_KIND_VTRANSFORM, d, A, Bm, C, 0);
+      e = cudaStreamSynchronize(ctx->stream);      // the descriptor tables are freed below
+      d.prob.release(); d.seg.release(); d.bucket.release();
+      if (rc) { cleanup(); return rc; }
+      if (e != cudaSuccess) { cleanup(); return cuda_fail(ctx, e, "block_maxabs"); }
+    }
+    std::vector<int> qkk((size_t)3 * ns);
+    for (long long l = 0; l < ns; ++l) {
+      int k1, k2, q, i1;
+      P.pair(s0 + l, k1, k2, q, i1);
+      qkk[3 * l] = q; qkk[3 * l + 1] = k2; qkk[3 * l + 2] = k1;
+    }
+    if ((rc = upload(ctx, d_qkk, qkk))) { cleanup(); return rc; }
+    e = launch_block_maxabs((const double2*)ctx->xbuf.p, (const int*)d_lab_aux.p, (const int*)d_lab_ao.p, (const int*)d_qkk.p,
+                            (double*)d_maxabs + (s0 - p0) * ncand, (int)ns, P.naux, P.nao, mb_aux, mb_ao, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { cleanup(); return cuda_fail(ctx, e, "block_maxabs reduction"); }
+    ctx->launches++;
+  }
+  cleanup();
+  return GWSIG_OK;
+}
+
 /* ---- N1: bare bubble P0^q(tau) (Eq. 20, Algorithm 3), dense modes ---------------------------- */
 int gwsig_p0_begin(gwsig_ctx* ctx, const void* dG, void* dP0, void* stream) {
   if (!ctx) return GWSIG_ERR_ARG;

@@ -297,6 +297,49 @@ cudaError_t launch_hartree(const double2* gamma, const double2* Vd, double2* rho
   return cudaGetLastError();
 }
 
+// Allowed-block detection ("only non-zero blocks are considered"): max |.| of every candidate block (p, alpha, iota)
+// of the block-basis tensors T3[pair][P][a][i] (Eq. 27).  One CTA per (pair, slab of auxiliary rows): a shared-memory table of the
+// pair's candidates (non-negative doubles order like their bit patterns: integer atomicMax), flushed to global once.
+__global__ void __launch_bounds__(256) block_maxabs_kernel(const double2* __restrict__ T3, const int* __restrict__ lab_aux, const int* __restrict__ lab_ao,
+                                                           const int* __restrict__ pair_qkk, unsigned long long* out, int naux, int nao, int mb_ao,
+                                                           int ncand, int rows_per_cta) {
+  extern __shared__ unsigned long long cand[];
+  const int pair = blockIdx.x, P0 = blockIdx.y * rows_per_cta, tid = threadIdx.x;
+  for (int c = tid; c < ncand; c += blockDim.x) cand[c] = 0ULL;
+  __syncthreads();
+  const int q = pair_qkk[3 * pair], k2 = pair_qkk[3 * pair + 1], k1 = pair_qkk[3 * pair + 2];
+  const int n2 = nao * nao;
+  const int P1 = min(naux, P0 + rows_per_cta);
+  const double2* T = T3 + (long long)pair * naux * n2;
+  for (long long e = (long long)P0 * n2 + tid; e < (long long)P1 * n2; e += blockDim.x) {
+    const int P = (int)(e / n2), ai = (int)(e - (long long)P * n2);
+    const int a = ai / nao, i = ai - a * nao;
+    const double2 v = T[e];
+    const double m = sqrt(v.x * v.x + v.y * v.y);
+    const int c = (lab_aux[q * naux + P] * mb_ao + lab_ao[k2 * nao + a]) * mb_ao + lab_ao[k1 * nao + i];
+    atomicMax(&cand[c], (unsigned long long)__double_as_longlong(m));
+  }
+  __syncthreads();
+  for (int c = tid; c < ncand; c += blockDim.x)
+    if (cand[c]) atomicMax(&out[(long long)pair * ncand + c], cand[c]);
+}
+
+cudaError_t launch_block_maxabs(const double2* T3, const int* lab_aux, const int* lab_ao, const int* pair_qkk, double* out, int npairs, int naux,
+                                int nao, int mb_aux, int mb_ao, cudaStream_t stream) {
+  if (npairs <= 0) return cudaSuccess;
+  const int ncand = mb_aux * mb_ao * mb_ao;
+  if ((size_t)ncand * sizeof(unsigned long long) > 48 * 1024) return cudaErrorInvalidValue;
+  const int rows_per_cta = 8;
+  for (int p0 = 0; p0 < npairs; p0 += 65535) {                     // (pairs on grid.x would do; kept symmetric with the other launchers)
+    const int np = std::min(65535, npairs - p0);
+    dim3 grid((unsigned)np, (unsigned)((naux + rows_per_cta - 1) / rows_per_cta));
+    block_maxabs_kernel<<<grid, 256, (size_t)ncand * sizeof(unsigned long long), stream>>>(T3 + (long long)p0 * naux * nao * nao, lab_aux, lab_ao,
+                                                                                           pair_qkk + 3LL * p0, (unsigned long long*)out + (long long)p0 * ncand,
+                                                                                           naux, nao, mb_ao, ncand, rows_per_cta);
+  }
+  return cudaGetLastError();
+}
+
 cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const double2* partial, double2* acc, int t0, cudaStream_t stream) {
   if (ngroups <= 0) return cudaSuccess;
   for (int g0 = 0; g0 < ngroups; g0 += 65535) {

@@ -759,14 +759,30 @@ int Plan::build_unfold(bool aux, int k_first, int k_count, int step, StagePlan& 
 
 int Plan::build_vtransform(long long p0, long long np, int step, StagePlan& out) const {
   out.prob.clear(); out.seg.clear(); out.bucket.clear(); out.ntiles = 0; out.red.clear(); out.partial_elems = 0;
-  if (mode != GWSIG_IBZ_BLOCK || !have_U || !have_triples) return GWSIG_ERR_ARG;
-  if (p0 < 0 || np < 1 || p0 + np > npairs || step < 1 || step > 3) return GWSIG_ERR_ARG;
+  // steps 1, 2: the dense transforms over the auxiliary and the first orbital index; step 3: the second orbital index, allowed
+  // triples only, written into the packed layout (needs set_triples); step 4: the second orbital index for EVERY block, dense
+  // (what the allowed-block detection looks at: gwsig_block_maxabs, before any triples exist)
+  if (mode != GWSIG_IBZ_BLOCK || !have_U || (step == 3 && !have_triples)) return GWSIG_ERR_ARG;
+  if (p0 < 0 || np < 1 || p0 + np > npairs || step < 1 || step > 4) return GWSIG_ERR_ARG;
   const long long n2 = (long long)nao * nao, xs = (long long)naux * n2;
   for (long long l = 0; l < np; ++l) {
     const long long p = p0 + l;
     int k1, k2, q, i1;
     pair(p, k1, k2, q, i1);
-    if (step < 3) {
+    if (step == 4) {          // T3[(P,a), i] = sum_j T2[P][a][j] U^{k1}[j, i]      (Eq. 27, last factor; no conjugation)
+      gwsig_seg S; std::memset(&S, 0, sizeof(S));
+      gwsig_problem P; std::memset(&P, 0, sizeof(P));
+      S.a_off = l * xs; P.c_off = l * xs;
+      S.am = lvl1(nao); S.ak = lvl1(1);
+      S.b_off = (long long)k1 * n2; S.bk = lvl1(nao); S.bn = lvl1(1);
+      S.K = nao;
+      P.M = naux * nao; P.N = nao;
+      P.cm = lvl1(nao); P.cn = lvl1(1);
+      P.flags = 0;
+      P.nbatch = 1;
+      P.seg_begin = (int)out.seg.size(); P.seg_count = 1;
+      out.seg.push_back(S); out.prob.push_back(P);
+    } else if (step < 3) {
       gwsig_seg S; std::memset(&S, 0, sizeof(S));
       gwsig_problem P; std::memset(&P, 0, sizeof(P));
       S.a_off = l * xs; P.c_off = l * xs;

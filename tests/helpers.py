@@ -328,3 +328,39 @@ def run_vtransform_numpy(cfg, inp, p0, npairs):
         pr, sg, _ = lib.plan_get(p0, npairs, 1, 40 + step)
         run_stage_numpy(pr, sg, A, Bm, C, 0)
     return out
+
+
+def oracle_block_maxabs(cfg, inp, pairs, mb_aux, mb_ao):
+    """max |.| of every candidate block (p, alpha, iota) of the Eq. 27 transform (oracle/block_oracle.py, dense) of the listed
+    pairs -> [len(pairs), mb_aux, mb_ao, mb_ao]; zero where a mesh point has fewer blocks."""
+    from oracle.block_oracle import block_transform_ref
+    lib = cfg.lib
+    out = np.zeros((len(pairs), mb_aux, mb_ao, mb_ao))
+    for n, p in enumerate(pairs):
+        k1, k2, q = lib.pair_info(p, with_layout=False)[:3]
+        T = block_transform_ref(inp.V2_rows(k1, [k2])[0], cfg.aux.U[q], cfg.ao.U[k2], cfg.ao.U[k1])
+        op, o2, o1 = cfg.aux.off[q], cfg.ao.off[k2], cfg.ao.off[k1]
+        for b in range(len(op) - 1):
+            for al in range(len(o2) - 1):
+                for io in range(len(o1) - 1):
+                    out[n, b, al, io] = np.abs(T[op[b]:op[b + 1], o2[al]:o2[al + 1], o1[io]:o1[io + 1]]).max()
+    return out
+
+
+def triples_from_maxabs(mx, thresh, vmax):
+    """allowed (p, alpha, iota) per pair from the block maxima, sorted by p, alpha, iota (the order symsetup.block_V2 uses)."""
+    return [np.argwhere(m > thresh * vmax).astype(np.int32) for m in mx]
+
+
+def run_dense_vtransform_numpy(cfg, inp, p0, npairs):
+    """launches 41, 42, 44 of gwsig_block_maxabs (the Eq. 27 transform for EVERY block, dense) with the numpy interpreter."""
+    lib = cfg.lib
+    xs = cfg.naux * cfg.nao ** 2
+    info = [lib.pair_info(p, with_layout=False) for p in range(p0, p0 + npairs)]
+    V = np.concatenate([inp.V2_rows(i[0], [i[1]])[0].ravel() for i in info])
+    Uaux, Uao = np.ascontiguousarray(cfg.aux.U).ravel(), np.ascontiguousarray(cfg.ao.U).ravel()
+    T1, T2, T3 = (np.zeros(npairs * xs, complex) for _ in range(3))
+    for step, (A, Bm, C) in zip((1, 2, 4), ((V, Uaux, T1), (T1, Uao, T2), (T2, Uao, T3))):
+        pr, sg, _ = lib.plan_get(p0, npairs, 1, 40 + step)
+        run_stage_numpy(pr, sg, A, Bm, C, 0)
+    return T3.reshape(npairs, cfg.naux, cfg.nao, cfg.nao)

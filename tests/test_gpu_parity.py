@@ -4,7 +4,8 @@ FP64, after folding the result back to the orbital basis."""
 import numpy as np
 import pytest
 
-from tests.helpers import fold_to_orbital, get_inputs, oracle_exchange, oracle_p0, oracle_packed_V, oracle_sigma, pack_V_p0, rel_err
+from tests.helpers import (fold_to_orbital, get_inputs, oracle_block_maxabs, oracle_exchange, oracle_p0, oracle_packed_V, oracle_sigma, pack_V_p0, rel_err,
+                           triples_from_maxabs)
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
@@ -352,6 +353,51 @@ def test_block_transform_v_eq27(name):
         ref = oracle_packed_V(cfg, inp, [p])
         assert np.abs(got[voff[p]:voff[p + 1]] - ref).max() <= 1e-13 * np.abs(dense).max()
     _check(cfg, inp, run_gpu(cfg, G, W, got), ks=None if inp.nk <= 64 else list(range(0, inp.nk, 7)))
+
+
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite", "cfg2"])
+def test_block_maxabs_device_prestep(name):
+    """N4, detection: gwsig_block_maxabs (Eq. 27 for every block + block maxima on the device, no triples set yet) against the
+    oracle's dense transform; its thresholded triples are the ones the CPU pre-step finds; the whole device pre-step
+    (detection -> set_triples -> gwsig_block_transform_v) then feeds a Sigma evaluation that matches the Sigma oracle."""
+    B = _B()
+    torch = _torch()
+    from paper_2405_09494_b200.pack import configure_from_crystal
+    inp = get_inputs(name)
+    lib = B.Gwsig(device=0)
+    cfg = configure_from_crystal(lib, inp.cr, 2, pass_U=True)
+    mb_aux = max(len(o) - 1 for o in cfg.aux.off) + 1                # one spare index each: unused candidates stay zero
+    mb_ao = max(len(o) - 1 for o in cfg.ao.off)
+    info = [lib.pair_info(p, with_layout=False) for p in range(cfg.npairs)]
+    dense = np.concatenate([inp.V2_rows(i[0], [i[1]])[0].ravel() for i in info])
+    dD = torch.from_numpy(dense).cuda()
+    dM = torch.full((cfg.npairs * mb_aux * mb_ao * mb_ao,), float("nan"), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    xs = inp.naux * inp.nao ** 2
+    third = cfg.npairs // 3
+    lib.block_maxabs(0, third, dD, mb_aux, mb_ao, dM, stream)                                  # two calls: a later pair range
+    lib.block_maxabs(third, cfg.npairs - third, dD[third * xs:], mb_aux, mb_ao, dM[third * mb_aux * mb_ao * mb_ao:], stream)
+    torch.cuda.synchronize()
+    got = dM.cpu().numpy().reshape(cfg.npairs, mb_aux, mb_ao, mb_ao)
+    vmax = np.abs(dense).max()
+    sample = list(range(0, cfg.npairs, max(1, cfg.npairs // 40)))
+    ref = oracle_block_maxabs(cfg, inp, sample, mb_aux, mb_ao)
+    assert np.abs(got[sample] - ref).max() <= 1e-12 * vmax
+    assert got[:, mb_aux - 1].max() == 0.0                                                     # the spare index was never touched
+    # forbidden blocks are zero to rounding, allowed ones are not: the threshold does not matter
+    assert not ((got > 1e-12 * vmax) & (got < 1e-6 * vmax)).any()
+    trip = triples_from_maxabs(got, 1e-9, vmax)
+    Vnp = cfg.pack_V(inp.V2_rows)                                    # CPU pre-step (symsetup.block_V2): its triples are the reference
+    assert all(np.array_equal(trip[p], cfg.triples[p]) for p in range(cfg.npairs))
+    # device pre-step end to end: the triples found on the device, then the packed transform on the device, then Sigma
+    tptr = np.zeros(cfg.npairs + 1, np.int64)
+    tptr[1:] = np.cumsum([len(t) for t in trip])
+    lib.set_triples(tptr, np.concatenate(trip))
+    dP = torch.full((Vnp.size,), float("nan"), dtype=torch.complex128, device="cuda")
+    lib.block_transform_v(0, cfg.npairs, dD, dP, stream)
+    torch.cuda.synchronize()
+    G, W = cfg.pack_GW(inp.G_k, lambda q: inp.W_full([q])[0])
+    _check(cfg, inp, run_gpu(cfg, G, W, dP.cpu().numpy()), ks=None if inp.nk <= 64 else list(range(0, inp.nk, 7)))
 
 
 @pytest.mark.parametrize("name,mode,nw", [("toy_wurtzite", 1, 3), ("cfg2", 1, 9), ("cfg1", 0, 7)])

@@ -250,6 +250,32 @@ def test_vtransform_plan_matches_oracle(name):
         lib.plan_get(0, 4, inp.ntau, 11)
 
 
+@pytest.mark.parametrize("name", ["toy_diamond4", "toy_wurtzite"])
+def test_dense_vtransform_plan_detects_the_allowed_blocks(name):
+    """N4: the launches of gwsig_block_maxabs (plan stages 41, 42, 44: the Eq. 27 transform for EVERY block), run
+    by the numpy interpreter BEFORE any triples are set, give the oracle's dense block-basis tensor; thresholding its block
+    maxima gives the triples the CPU pre-step (symsetup.block_V2) finds."""
+    from oracle.block_oracle import block_transform_ref
+    from tests.helpers import run_dense_vtransform_numpy
+    inp = make_inputs(name)
+    lib = B.Gwsig(device=-1)
+    cfg = configure_from_crystal(lib, inp.cr, B.IBZ_BLOCK, pass_U=True)
+    p0, n = 3, 9
+    got = run_dense_vtransform_numpy(cfg, inp, p0, n)
+    with pytest.raises(B.GwsigError):                      # the packed step 3 needs the triples
+        lib.plan_get(p0, n, 1, 43)
+    for l in range(n):
+        k1, k2, q = lib.pair_info(p0 + l, with_layout=False)[:3]
+        V2 = inp.V2_rows(k1, [k2])[0]
+        ref = block_transform_ref(V2, cfg.aux.U[q], cfg.ao.U[k2], cfg.ao.U[k1])
+        assert np.abs(got[l] - ref).max() < 1e-13 * np.abs(ref).max()
+        trip, _ = cfg.setup.block_V2(V2, k1, k2, cfg.ao, cfg.aux)
+        op, o2, o1 = cfg.aux.off[q], cfg.ao.off[k2], cfg.ao.off[k1]
+        mine = [(b, al, io) for b in range(len(op) - 1) for al in range(len(o2) - 1) for io in range(len(o1) - 1)
+                if np.abs(got[l][op[b]:op[b + 1], o2[al]:o2[al + 1], o1[io]:o1[io + 1]]).max() > 1e-9 * np.abs(got[l]).max()]
+        assert mine == [tuple(t) for t in trip]
+
+
 def test_gridtransform_plan_matches_einsum():
     """N3 (Eq. 19): the tau <-> i Omega transform descriptors (plan stage 51), run by the numpy interpreter, are the einsum."""
     from tests.helpers import run_stage_numpy
