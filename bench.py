@@ -56,6 +56,9 @@ def parse_args():
     ap.add_argument("--engine", type=int, default=0, choices=[0, 2, 3], help="0: per-stage choice (default), 2: DMMA 4M kernel, 3: DMMA 3M kernel")
     ap.add_argument("--scratch-mib", type=int, default=0, help="main leg only: cap of the X + Y scratch in MiB (0: library default, 8192); small values "
                     "give chunks that stay in L2 at the price of many short launches (experiments)")
+    ap.add_argument("--prestep", default="library", choices=["library", "torch"],
+                    help="IBZ_BLOCK preparation of V (Eq. 27 transform, allowed-block detection, packing): the library's own calls "
+                         "gwsig_block_maxabs / gwsig_block_transform_v (default) or the torch pre-step of presetup_device.py")
     ap.add_argument("--probe-only", action="store_true", help="print the FP64 issue-rate probes and exit")
     return ap.parse_args()
 
@@ -147,10 +150,11 @@ class Workload:
     on demand": here it is re-derived on demand from the compact real-space table)."""
 
     def __init__(self, name, mode, B, pack, inp=None, nq_subset=None, torch=None, dev=None, device_index=0, host_only=False,
-                 resident_limit_gb=110.0, q_per_batch=None, dv=None):
+                 resident_limit_gb=110.0, q_per_batch=None, dv=None, prestep="library"):
         from gwsig_synth import make_inputs
         self.name, self.mode, self.torch, self.dev = name, mode, torch, dev
         self.dv = dv                  # the device copy of the real-space V table is shared by the legs of a run (93 GiB at cfg5)
+        self.lib_prestep = prestep == "library" and mode == B.IBZ_BLOCK and torch is not None and name != "cfg1" and not host_only
         self.inp = inp if inp is not None else make_inputs(name)
         inp = self.inp
         self.lib = B.Gwsig(device=-1 if host_only else device_index)
@@ -165,7 +169,8 @@ class Workload:
             nq_ = cr.kmesh.nk if nq_subset is None else nq_subset          # W(q) of q slices that are never pushed is never read
             G_of, W_of = inp.G_k, (lambda q: inp.W_full([q])[0])
         else:
-            self.cfg = pack.configure_from_crystal(self.lib, inp.cr, mode)
+            # the library's Eq. 27 calls need the adapted bases U handed to set_blocks (gauge S5 is recognised: no unfold is planned)
+            self.cfg = pack.configure_from_crystal(self.lib, inp.cr, mode, pass_U=self.lib_prestep)
             G_of, W_of = inp.G_k, (lambda q: inp.W_full([q])[0])
         cfg = self.cfg
         if nq_ is not None and nq_ < cfg.nk:
@@ -205,8 +210,12 @@ class Workload:
         self.batches = [(q0 * nk1, min(q0 + qb, self.nq) * nk1) for q0 in range(0, self.nq, qb)]
         blockmode = self.mode == B.IBZ_BLOCK
         if blockmode:
-            from paper_2405_09494_b200.presetup_device import DeviceBlocker
-            self.blk = DeviceBlocker(cfg, torch, dev)
+            if not self.lib_prestep:
+                from paper_2405_09494_b200.presetup_device import DeviceBlocker
+                self.blk = DeviceBlocker(cfg, torch, dev)
+            else:
+                mb_aux = max(len(o) - 1 for o in cfg.aux.off)
+                mb_ao = max(len(o) - 1 for o in cfg.ao.off)
             # pass 1 (pre-step, all pairs of the mode: set_triples wants every pair): allowed blocks by block max-abs
             trip, vmax = [], None
             allb = [(q0 * nk1, min(q0 + qb, cfg.nk) * nk1) for q0 in range(0, cfg.nk, qb)]
@@ -216,21 +225,34 @@ class Workload:
                 if bi == 0:
                     self.dv.check(k2s, k1s, V)
                     vmax = float(V.abs().max())
-                T = self.blk.transform(V.reshape(len(k1s), cfg.naux, cfg.nao, cfg.nao), qs, k2s, k1s)
-                del V
-                trip += self.blk.triples_from_maxabs(self.blk.block_maxabs(T, qs, k2s, k1s), qs, k2s, k1s, 1e-9, vmax)
-                del T
+                if self.lib_prestep:
+                    # Eq. 27 for every block + block maxima in the library (gwsig_block_maxabs), thresholded here
+                    dM = torch.empty((p1 - p0, mb_aux, mb_ao, mb_ao), dtype=torch.float64, device=dev)
+                    lib.block_maxabs(p0, p1 - p0, V.contiguous(), mb_aux, mb_ao, dM, torch.cuda.current_stream().cuda_stream)
+                    mx = dM.cpu().numpy()
+                    trip += [np.argwhere(m > 1e-9 * vmax).astype(np.int32) for m in mx]
+                    del V, dM
+                else:
+                    T = self.blk.transform(V.reshape(len(k1s), cfg.naux, cfg.nao, cfg.nao), qs, k2s, k1s)
+                    del V
+                    trip += self.blk.triples_from_maxabs(self.blk.block_maxabs(T, qs, k2s, k1s), qs, k2s, k1s, 1e-9, vmax)
+                    del T
             tptr = np.zeros(cfg.npairs + 1, np.int64)
             tptr[1:] = np.cumsum([len(t) for t in trip])
             lib.set_triples(tptr, np.concatenate(trip))
             cfg.triple_ptr, cfg.triples = tptr, trip
-            self.tables = []
-            for (p0, p1) in self.batches:
-                qs, k2s, k1s = self._pairs(p0, p1)
-                self.tables.append(self.blk.pack_tables(trip[p0:p1], qs, k2s, k1s))
-            sizes = np.concatenate([t[3] for t in self.tables])
-            assert all(int(sizes[i]) == lib.pair_info(i)[4] for i in (0, len(sizes) // 2, len(sizes) - 1)), "packed V layout mismatch"
-            self.voff = np.concatenate([[0], np.cumsum(sizes)])
+            if self.lib_prestep:
+                self.voff = np.array([lib.pair_info(p)[3] for p in range(self.npairs_run)] + [0], np.int64)
+                last = lib.pair_info(self.npairs_run - 1)
+                self.voff[-1] = last[3] + last[4]
+            else:
+                self.tables = []
+                for (p0, p1) in self.batches:
+                    qs, k2s, k1s = self._pairs(p0, p1)
+                    self.tables.append(self.blk.pack_tables(trip[p0:p1], qs, k2s, k1s))
+                sizes = np.concatenate([t[3] for t in self.tables])
+                assert all(int(sizes[i]) == lib.pair_info(i)[4] for i in (0, len(sizes) // 2, len(sizes) - 1)), "packed V layout mismatch"
+                self.voff = np.concatenate([[0], np.cumsum(sizes)])
         else:
             self.voff = np.arange(self.npairs_run + 1, dtype=np.int64) * nel
         total_gb = float(self.voff[-1]) * 16 / 1e9
@@ -253,7 +275,11 @@ class Workload:
         V = self.dv.dense(k2s, k1s)
         if check:
             self.dv.check(k2s, k1s, V)
-        if self.mode == 2:
+        if self.mode == 2 and self.lib_prestep:
+            # Eq. 27 on the allowed blocks, written straight into the packed layout by the library (gwsig_block_transform_v)
+            self.lib.block_transform_v(p0, p1 - p0, V.contiguous(), dst[base:], self.torch.cuda.current_stream().cuda_stream)
+            del V
+        elif self.mode == 2:
             cfg = self.cfg
             T = self.blk.transform(V.reshape(len(k1s), cfg.naux, cfg.nao, cfg.nao), qs, k2s, k1s)
             del V
@@ -546,7 +572,7 @@ def main():
     if args.workload == "cfg1":
         mode = B.FULL_BZ
     t_setup = time.time()
-    wl = Workload(args.workload, mode, B, pack, torch=torch, dev=dev, device_index=local)
+    wl = Workload(args.workload, mode, B, pack, torch=torch, dev=dev, device_index=local, prestep=args.prestep)
     cfg, lib = wl.cfg, wl.lib
     lib.set_option("engine", args.engine)
     if args.scratch_mib > 0:
@@ -698,7 +724,7 @@ def main():
         dG = dW = dS = None
         torch.cuda.empty_cache()
         t4 = time.time()
-        w4 = Workload("cfg4", MODES[args.mode], B, pack, torch=torch, dev=dev, device_index=local)
+        w4 = Workload("cfg4", MODES[args.mode], B, pack, torch=torch, dev=dev, device_index=local, prestep=args.prestep)
         w4.lib.set_option("engine", args.engine)
         tt, k4, l4, dS4 = run_steps(w4, torch, dev, 1, 1, timing=True)
         sf4 = stage_flops(w4, B)

@@ -230,7 +230,9 @@ int gwsig_dyson_solve_noalloc(const void* dA, void* dX, int nmat, int n, void* d
  * order, dV_packed (dev) receives the allowed blocks in the packed layout sigma_push_pairs expects (first element = first
  * element of pair p0).  Needs GWSIG_IBZ_BLOCK, set_blocks WITH U_ao / U_aux, set_triples.  Three launches of the grouped engine
  * per sub-batch of pairs (auxiliary index, first orbital index, second orbital index + packing); the paper does this step on
- * the CPU before the calculation.  Synchronises the stream.                                              */
+ * the CPU before the calculation.  Synchronises the stream.                                              
+ * May be called between the gwsig_sigma_push_pairs calls of an open Sigma evaluation (V prepared on demand) if `stream`
+ * is that evaluation's stream; not while a P0 evaluation is open.  */
 int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_dense, void* dV_packed, void* stream);
 
 /* ---- N4, second half: allowed-block detection on the device ("only non-zero blocks are considered") ----

@@ -862,7 +862,10 @@ int gwsig_block_transform_v(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* 
   if (P.mode != GWSIG_IBZ_BLOCK || !P.have_blocks || !P.have_triples)
     return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: needs GWSIG_IBZ_BLOCK with set_blocks and set_triples");
   if (!P.have_U) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: set_blocks must be given the adapted bases U_ao, U_aux");
-  if (ctx->in_eval || ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "block_transform_v: an evaluation is open");
+  // V prepared on demand ("copied on demand"): the call is allowed between the pushes of an open Sigma evaluation,
+  // on that evaluation's stream (it shares the X / Y scratch and the tile counters with it, in stream order)
+  if (ctx->in_p0) return fail(ctx, GWSIG_ERR_ORDER, "block_transform_v: a P0 evaluation is open");
+  if (ctx->in_eval && (cudaStream_t)stream != ctx->stream) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: inside an open evaluation the stream must be the evaluation's");
   if (np < 1 || p0 < 0 || p0 + np > P.npairs) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: bad pair range");
   if (!dV_dense || !dV_packed) return fail(ctx, GWSIG_ERR_ARG, "block_transform_v: NULL device pointer");
   int rc = ensure_cuda(ctx);
