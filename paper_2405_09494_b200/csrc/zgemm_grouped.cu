@@ -128,7 +128,7 @@ __device__ __forceinline__ TileInfo decode_tile(const ZgParams& p, long long til
   return t;
 }
 
-struct SlotHdr {
+struct __align__(16) SlotHdr {
   int ctl;            // bit0: first slot of a tile, bit1: last slot of a tile, bit2: no more work
   int nk4;            // k4-steps of this slot that hold data (1 or 2)
   int trec;           // index of the tile record (valid when bit0)
@@ -718,16 +718,18 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
 // double as the P1 / P2 operands (sign flips in place), only the operand sums of P3 need registers of their own, so the warp
 // stays inside the 96 registers a 20-warp CTA gives every thread; P1 is issued before the operand sums so that the FP64 adds
 // queue behind the warp's own DMMAs, and the other three warps of the sub-partition cover the fragment-load latency.
-template <int NI>
+template <int NI, bool kFlip>
 __device__ __forceinline__ void mma3_slot(double (&acc)[4][3][2], const double2* as, const double2* bs, int nk4, unsigned sa, unsigned sb) {
 #pragma unroll 1
   for (int kk = 0; kk < nk4; ++kk) {
     double2 af = as[kk * 4 * LDA3], bf[NI];
 #pragma unroll
     for (int j = 0; j < NI; ++j) bf[j] = bs[kk * 4 * LDB + j * 8];
-    af.y = xor_hi(af.y, sa);
+    if (kFlip) {                       // conj(A) / conj(B): stage 2 has neither, and five XORs per 12 DMMA are issue slots
+      af.y = xor_hi(af.y, sa);
 #pragma unroll
-    for (int j = 0; j < NI; ++j) bf[j].y = xor_hi(bf[j].y, sb);
+      for (int j = 0; j < NI; ++j) bf[j].y = xor_hi(bf[j].y, sb);
+    }
 #pragma unroll
     for (int j = 0; j < NI; ++j) dmma884(acc[j][0][0], acc[j][0][1], af.x, bf[j].x);
     const double asum = af.x + af.y;
@@ -810,10 +812,11 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
     unsigned phase = 0, sa = 0, sb = 0;
     while (true) {
       mbar_wait(full0 + 8 * stage, phase);
-      const int ctl = hdr[stage].ctl;
+      const int4 h4 = *reinterpret_cast<const int4*>(&hdr[stage]);      // ctl, nk4, trec in one 16-byte load
+      const int ctl = h4.x;
       if (ctl & 4) break;
       if (ctl & 1) {
-        tslot = hdr[stage].trec;
+        tslot = h4.z;
         const TileRec& t = trec[tslot];
         active = warp * 8 < t.mrows;
         ng = (t.ncols + 7) >> 3;
@@ -827,11 +830,18 @@ __global__ void __launch_bounds__(kThreads3, 2) zgemm_grouped_dmma3m(ZgParams p)
       if (active) {
         const double2* as = As + stage * BK3 * LDA3 + fk * LDA3 + warp * 8 + fr;
         const double2* bs = Bs + stage * BK3 * LDB + fk * LDB + zg_bcol(fr);
-        const int nk4 = hdr[stage].nk4;
-        if (ng == 4) mma3_slot<4>(acc, as, bs, nk4, sa, sb);
-        else if (ng == 3) mma3_slot<3>(acc, as, bs, nk4, sa, sb);
-        else if (ng == 2) mma3_slot<2>(acc, as, bs, nk4, sa, sb);
-        else mma3_slot<1>(acc, as, bs, nk4, sa, sb);
+        const int nk4 = h4.y;
+        if (sa | sb) {
+          if (ng == 4) mma3_slot<4, true>(acc, as, bs, nk4, sa, sb);
+          else if (ng == 3) mma3_slot<3, true>(acc, as, bs, nk4, sa, sb);
+          else if (ng == 2) mma3_slot<2, true>(acc, as, bs, nk4, sa, sb);
+          else mma3_slot<1, true>(acc, as, bs, nk4, sa, sb);
+        } else {
+          if (ng == 4) mma3_slot<4, false>(acc, as, bs, nk4, sa, sb);
+          else if (ng == 3) mma3_slot<3, false>(acc, as, bs, nk4, sa, sb);
+          else if (ng == 2) mma3_slot<2, false>(acc, as, bs, nk4, sa, sb);
+          else mma3_slot<1, false>(acc, as, bs, nk4, sa, sb);
+        }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(empty0 + 8 * stage);
