@@ -488,6 +488,19 @@ def sample_points(cfg_ir_list, ntau, nk_sample, ntau_sample):
     return ks, taus
 
 
+def replicas_step_time(secs_local, steps, world, dist=None, torch=None, device=None):
+    """the N > 1 rule of this bench (replicas only, no data-path collective): every rank evaluates the
+    same Sigma on its own GPU; the step time is the MAX over ranks of the device-timed region (one all_reduce of one double),
+    and `world` evaluations finish per step, so the whole-job metric is step time / world.  Returns (ms_per_step, ms_per_evaluation)."""
+    secs = float(secs_local)
+    if world > 1:
+        t = torch.tensor([secs], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        secs = float(t.item())
+    ms_step = secs / steps * 1e3
+    return ms_step, ms_step / world
+
+
 def reference_main(args, rank, world):
     """--impl reference: the oracle as it stands on the host cores, on a bounded sample of the same workload."""
     if rank != 0:
@@ -599,14 +612,9 @@ def main():
     clocks = sampler.stop()
     kinds = lib.kernel_times()
     launches = lib.last_launch_count()
-    if world > 1:
-        t = torch.tensor([secs], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        secs = float(t.item())
+    ms_step, ms_eval = replicas_step_time(secs, args.steps, world, dist, torch, dev)     # max over ranks; `world` evaluations per step
     sigma_gpu = dS.cpu().numpy()
     dV = None
-    ms_step = secs / args.steps * 1e3
-    ms_eval = ms_step / world                      # replicas: `world` evaluations finish per step time
 
     line = {"metric": METRIC, "value": ms_eval, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
