@@ -48,9 +48,12 @@ __device__ __forceinline__ long long idx2(const gwsig_idx2& d, int i) {
   return (long long)q * d.hi + (long long)r * d.lo;
 }
 
+// 16-byte asynchronous copy global -> shared; !valid writes 16 zero bytes and reads nothing (the ignore-src predicate form: one
+// LDGSTS; with a variable src-size operand ptxas spends six more instructions per copy on the size arithmetic)
 __device__ __forceinline__ void cp_async16(unsigned smem_dst, const void* gmem_src, bool valid) {
-  int bytes = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gmem_src), "r"(bytes) : "memory");
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.eq.b32 p, %2, 0;\n\tcp.async.cg.shared.global [%0], [%1], 16, p;\n\t}\n" ::"r"(smem_dst), "l"(gmem_src),
+               "r"((int)valid)
+               : "memory");
 }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
   asm volatile("mbarrier.init.shared.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
@@ -502,7 +505,7 @@ __device__ __forceinline__ void kstep_next(KStep& s) {        // branch-free: di
   s.r = w ? 0 : s.r;
 }
 __device__ __forceinline__ void cp_async16_sz(unsigned smem_dst, const void* gmem_src, unsigned bytes) {   // bytes = 0: zero-fill, no read
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gmem_src), "r"(bytes) : "memory");
+  cp_async16(smem_dst, gmem_src, bytes != 0u);
 }
 
 // per loader warp: the descriptor of the problem its tile ids are running through and the segment being staged, copied to
@@ -657,6 +660,28 @@ __device__ __forceinline__ void loader3(const ZgParams& p, double2* As, double2*
                 cp_async16_sz(brow, qb, kok ? szb : 0u);
                 arow += (unsigned)LDA3 * 16u; brow += (unsigned)LDB * 16u;
                 if (kok) { qa0 += sa_; qa1 += sa_; qb += sb_; }       // (never step past the last row: the pointers stay valid)
+              }
+              mbar_arrive_cp_async(bar_full);
+              continue;
+            }
+            if (!a_row && !b_row && ak.div == bk.div) {
+              // stage 3 (and every pair of operands cut from the same [P'][b][.] layout): A and B step through k with the SAME
+              // fast-index period, so one (quotient, remainder) walk serves both offsets
+              KStep ka = kstep_init(ak, k0);
+              long long offb = ak.div == GWSIG_NODIV ? (long long)k0 * bk.lo : (long long)(k0 / ak.div) * bk.hi + (long long)(k0 % ak.div) * bk.lo;
+              const long long wrapb = ak.div == GWSIG_NODIV ? 0 : bk.hi - (long long)bk.div * bk.lo;
+              unsigned arow = as + (unsigned)lane * 16u, brow = bs + (unsigned)lane * 16u;
+#pragma unroll 4
+              for (int kk = 0; kk < 4 * nk4; ++kk) {
+                const bool kok = kk < nkv;
+                cp_async16_sz(arow, pa[0] + ka.off, kok ? sza[0] : 0u);
+                cp_async16_sz(arow + 32u * 16u, pa[1] + ka.off, kok ? sza[1] : 0u);
+                cp_async16_sz(brow, pb + offb, kok ? szb : 0u);
+                arow += (unsigned)LDA3 * 16u; brow += (unsigned)LDB * 16u;
+                const bool w = ++ka.r == ka.div;
+                ka.off += ka.lo + (w ? ka.wrap : 0);
+                offb += bk.lo + (w ? wrapb : 0);
+                ka.r = w ? 0 : ka.r;
               }
               mbar_arrive_cp_async(bar_full);
               continue;
