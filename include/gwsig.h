@@ -255,6 +255,7 @@ int gwsig_block_maxabs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV_de
  * uniform on [0, beta]: G(-tau_n) = -G(beta - tau_n) = -G[ntau-1-n].
  *   dG   : as for sigma_begin (wedge data in IBZ mode, unfolded by Eq. 22)
  *   dV   : T = V^{k,k+q}_{Q,da} as [naux][nao][nao] per pair, pairs ordered k-major: pair = k * nq + iq, q = q_list[iq]
+ *          (each push is copied once into the layout [nao][nao][naux] -- auxiliary index last -- which stages 1 and 2 address)
  *          (gwsig_get_ibz / set_output_points give the list), k over the whole mesh; the partner V^{k+q,k} is taken as the
  *          conjugate transpose (reading A7 of DESIGN.md)
  *   dP0  : [nq][ntau][naux][naux], written by p0_end

@@ -77,6 +77,7 @@ struct gwsig_ctx {
   DevBuf oblk_ao, oblk_aux, unf_tmp, partial;
   DevBuf dys_flag;                               // N3: singular-matrix flag of the Eq. 19 solve
   DevBuf hart_rho;                               // N2: auxiliary density rho_Q of the Hartree term (Eq. 21b)
+  DevBuf p0vt;                                   // N1: aux-last copy T'[x][y][Q] of the pushed pair tensors (stages 1, 2 of Algorithm 3)
   DevBuf u_ao_dev, u_aux_dev;                    // N4: the adapted bases on the device (set_blocks with U)
   DevBuf grev, p0acc, p0desc;                    // N1 (Eq. 20): G(beta - tau) on the full zone, the P0 accumulator, its epilogue descriptors
   bool in_p0 = false;
@@ -382,7 +383,7 @@ int gwsig_destroy(gwsig_ctx* ctx) {
   if (ctx->cuda_ready) {
     cudaSetDevice(ctx->device);
     DevBuf* bufs[] = {&ctx->gbz, &ctx->wring, &ctx->xbuf, &ctx->ybuf, &ctx->sigacc, &ctx->counters, &ctx->epidesc,
-                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->dys_flag, &ctx->hart_rho, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
+                      &ctx->probe_sink, &ctx->oblk_ao, &ctx->oblk_aux, &ctx->unf_tmp, &ctx->partial, &ctx->grev, &ctx->p0acc, &ctx->p0desc, &ctx->u_ao_dev, &ctx->u_aux_dev, &ctx->dys_flag, &ctx->hart_rho, &ctx->p0vt, &ctx->tgt_src, &ctx->tgt_op, &ctx->colphase_ao, &ctx->ell_cols_ao,
                       &ctx->ell_vals_ao, &ctx->ell_cnt_ao, &ctx->wtgt_src, &ctx->wtgt_op, &ctx->colphase_aux,
                       &ctx->ell_cols_aux, &ctx->ell_vals_aux, &ctx->ell_cnt_aux, &ctx->h_g, &ctx->h_w, &ctx->h_sig,
                       &ctx->h_vslot[0], &ctx->h_vslot[1]};
@@ -1014,11 +1015,15 @@ int gwsig_p0_begin(gwsig_ctx* ctx, const void* dG, void* dP0, void* stream) {
   if (rc) return rc;
   const double2* Gsrc = P.mode == GWSIG_IBZ ? (const double2*)ctx->gbz.p : ctx->dG;
   const long long n2 = (long long)P.nao * P.nao;
-  CU(ctx->grev.ensure((size_t)P.nk * P.ntau * n2 * sizeof(double2)));
-  // G(-tau_n) = -G(beta - tau_n) = -G[ntau-1-n] (fermionic antiperiodicity, uniform grid): the reversed copy; the sign goes
-  // into the epilogue (-(1/Nk) of Eq. 20 becomes +1/Nk)
-  CU(launch_reverse_tau(Gsrc, (double2*)ctx->grev.p, P.nk, P.ntau, n2, ctx->stream));
-  ctx->launches++;
+  // two transposed copies of G on the whole zone (Algorithm 3 contracts G over its second index: the transposes make the tile
+  // rows the contiguous index of the A operand): grev[0 .. ) = G(beta - tau)^T and, behind it, G(tau)^T.
+  // G(-tau_n) = -G(beta - tau_n) = -G[ntau-1-n] (fermionic antiperiodicity, uniform grid); the sign goes into the epilogue
+  // (-(1/Nk) of Eq. 20 becomes +1/Nk)
+  const size_t gelems = (size_t)P.nk * P.ntau * n2;
+  CU(ctx->grev.ensure(2 * gelems * sizeof(double2)));
+  CU(launch_transpose_tau(Gsrc, (double2*)ctx->grev.p, P.nk, P.ntau, P.nao, true, ctx->stream));
+  CU(launch_transpose_tau(Gsrc, (double2*)ctx->grev.p + gelems, P.nk, P.ntau, P.nao, false, ctx->stream));
+  ctx->launches += 2;
   const size_t pe = (size_t)P.nk1 * P.ntau * P.naux * P.naux;
   CU(ctx->p0acc.ensure(std::max<size_t>(pe * sizeof(double2), 16)));
   CU(cudaMemsetAsync(ctx->p0acc.p, 0, pe * sizeof(double2), ctx->stream));
@@ -1055,7 +1060,11 @@ int gwsig_p0_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV) 
     const size_t xbytes = (size_t)xs * ns * nt * sizeof(double2);
     CU(ctx->xbuf.ensure(xbytes));
     CU(ctx->ybuf.ensure(xbytes));
-    const double2* Vsub = Vbase + (s0 - p0) * xs;
+    // the sub-batch's pair tensors with the auxiliary index last (what the stage-1 / stage-2 descriptors address)
+    CU(ctx->p0vt.ensure((size_t)xs * ns * sizeof(double2)));
+    CU(launch_aux_last(Vbase + (s0 - p0) * xs, (double2*)ctx->p0vt.p, ns, P.naux, P.nao * P.nao, ctx->stream));
+    ctx->launches++;
+    const double2* Vsub = (const double2*)ctx->p0vt.p;
     for (int t0 = 0; t0 < P.ntau; t0 += nt) {
       const int ntc = std::min(nt, P.ntau - t0);
       auto key = std::make_tuple((long long)s0, (long long)ns, ntc);
@@ -1079,7 +1088,7 @@ int gwsig_p0_push_pairs(gwsig_ctx* ctx, int64_t p0, int64_t np, const void* dV) 
       }
       int rc;
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE1, dp->st[0], (const double2*)ctx->grev.p, Vsub, (double2*)ctx->xbuf.p, t0))) return rc;   // X1
-      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], Gsrc, Vsub, (double2*)ctx->ybuf.p, t0))) return rc;                          // X2
+      if ((rc = run_stage(ctx, GWSIG_KIND_STAGE2, dp->st[1], (const double2*)ctx->grev.p + (size_t)P.nk * P.ntau * P.nao * P.nao, Vsub, (double2*)ctx->ybuf.p, t0))) return rc;   // X2
       if ((rc = run_stage(ctx, GWSIG_KIND_STAGE3, dp->st[2], (const double2*)ctx->xbuf.p, (const double2*)ctx->ybuf.p, (double2*)ctx->p0acc.p, t0))) return rc;
     }
     s0 += ns;

@@ -155,17 +155,24 @@ cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_
   return cudaGetLastError();
 }
 
-__global__ void __launch_bounds__(256) reverse_tau_kernel(const double2* src, double2* dst, int ntau, long long elems) {
+// P0 (Eq. 20): dst[k][n] = src[k][reverse ? ntau-1-n : n]^T for square matrices of side nao.  Stages 1 and 2 of Algorithm 3
+// contract G over its SECOND index (X1 = sum_d G[c,d] T[d,..]); the transposed copy makes the tile rows (c) the contiguous index
+// of the A operand, as in stage 1 of the Sigma path.  One CTA per (k, tau); the matrices are small (nao <= a few hundred).
+__global__ void __launch_bounds__(256) transpose_tau_kernel(const double2* src, double2* dst, int ntau, int nao, int reverse) {
   const long long kt = blockIdx.x;                       // k * ntau + n   (grid.x: Nk * ntau exceeds 65535 at config 5)
   const long long k = kt / ntau, n = kt % ntau;
-  const double2* s_ = src + (k * ntau + (ntau - 1 - n)) * elems;
+  const long long elems = (long long)nao * nao;
+  const double2* s_ = src + (k * ntau + (reverse ? ntau - 1 - n : n)) * elems;
   double2* d_ = dst + kt * elems;
-  for (long long e = threadIdx.x; e < elems; e += blockDim.x) d_[e] = s_[e];
+  for (long long e = threadIdx.x; e < elems; e += blockDim.x) {
+    const int r = (int)(e / nao), c = (int)(e - (long long)r * nao);
+    d_[e] = s_[(long long)c * nao + r];
+  }
 }
 
-cudaError_t launch_reverse_tau(const double2* src, double2* dst, int nk, int ntau, long long elems, cudaStream_t stream) {
+cudaError_t launch_transpose_tau(const double2* src, double2* dst, int nk, int ntau, int nao, bool reverse, cudaStream_t stream) {
   if (nk <= 0 || ntau <= 0) return cudaSuccess;
-  reverse_tau_kernel<<<(unsigned)((long long)nk * ntau), 256, 0, stream>>>(src, dst, ntau, elems);
+  transpose_tau_kernel<<<(unsigned)((long long)nk * ntau), 256, 0, stream>>>(src, dst, ntau, nao, reverse ? 1 : 0);
   return cudaGetLastError();
 }
 
@@ -336,6 +343,34 @@ cudaError_t launch_block_maxabs(const double2* T3, const int* lab_aux, const int
     block_maxabs_kernel<<<grid, 256, (size_t)ncand * sizeof(unsigned long long), stream>>>(T3 + (long long)p0 * naux * nao * nao, lab_aux, lab_ao,
                                                                                            pair_qkk + 3LL * p0, (unsigned long long*)out + (long long)p0 * ncand,
                                                                                            naux, nao, mb_ao, ncand, rows_per_cta);
+  }
+  return cudaGetLastError();
+}
+
+// P0 (Eq. 20): the pair tensors arrive as T[Q][x][y] (auxiliary index first, like every dense V of the interface); stages 1 and 2
+// of Algorithm 3 want the auxiliary index LAST -- T'[x][y][Q] -- so that both the tile rows of X1 / X2 and the operand rows they are
+// made from are contiguous in Q.  One tiled transpose [naux][nao^2] -> [nao^2][naux] per pair per push (read + write of V once).
+__global__ void __launch_bounds__(256) aux_last_kernel(const double2* __restrict__ src, double2* __restrict__ dst, int naux, int n2) {
+  __shared__ double2 tile[32][33];
+  const long long base = (long long)blockIdx.z * naux * n2;
+  const int x0 = blockIdx.x * 32, q0 = blockIdx.y * 32;            // x = (x, y) flattened, q = auxiliary index
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;          // 32 x 8 threads
+  for (int j = ty; j < 32; j += 8) {
+    const int q = q0 + j, x = x0 + tx;
+    if (q < naux && x < n2) tile[j][tx] = src[base + (long long)q * n2 + x];
+  }
+  __syncthreads();
+  for (int j = ty; j < 32; j += 8) {
+    const int x = x0 + j, q = q0 + tx;
+    if (q < naux && x < n2) dst[base + (long long)x * naux + q] = tile[tx][j];
+  }
+}
+
+cudaError_t launch_aux_last(const double2* src, double2* dst, long long npairs, int naux, int n2, cudaStream_t stream) {
+  for (long long p0 = 0; p0 < npairs; p0 += 65535) {
+    const int np = (int)std::min<long long>(65535, npairs - p0);
+    dim3 grid((unsigned)((n2 + 31) / 32), (unsigned)((naux + 31) / 32), (unsigned)np);
+    aux_last_kernel<<<grid, 256, 0, stream>>>(src + p0 * (long long)naux * n2, dst + p0 * (long long)naux * n2, naux, n2);
   }
   return cudaGetLastError();
 }

@@ -38,10 +38,11 @@ cudaError_t launch_reduce_parts(const RedGroupDev* groups, int ngroups, const do
 // Eq. 19a per matrix: X <- [1 - X]^{-1} X in place, nmat matrices [n][n] back to back; work = per-CTA scratch [ncta][n][2n]
 cudaError_t launch_block_maxabs(const double2* T3, const int* lab_aux, const int* lab_ao, const int* pair_qkk, double* out, int npairs, int naux,
                                 int nao, int mb_aux, int mb_ao, cudaStream_t stream);
+cudaError_t launch_aux_last(const double2* src, double2* dst, long long npairs, int naux, int n2, cudaStream_t stream);
 cudaError_t launch_hartree(const double2* gamma, const double2* Vd, double2* rho, double2* J, int nk, int nao, int naux, cudaStream_t stream);
 cudaError_t launch_dyson_solve(double2* X, int nmat, int n, double2* work, int ncta, int* fail_flag, cudaStream_t stream);
 // dst[k][n] = src[k][ntau-1-n] for nk matrices-over-tau of `elems` complex numbers each (G(beta - tau) for Eq. 20)
-cudaError_t launch_reverse_tau(const double2* src, double2* dst, int nk, int ntau, long long elems, cudaStream_t stream);
+cudaError_t launch_transpose_tau(const double2* src, double2* dst, int nk, int ntau, int nao, bool reverse, cudaStream_t stream);
 cudaError_t launch_unfold_sparse(const UnfoldParams& p, int ntarget, cudaStream_t stream);
 cudaError_t launch_epilogue(const EpilogueParams& p, int ndesc, int num_sms, cudaStream_t stream);
 cudaError_t launch_probe(int kind, int warps_per_block, int blocks, long long iters, double* sink, cudaStream_t stream,

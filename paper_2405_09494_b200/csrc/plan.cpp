@@ -910,11 +910,11 @@ int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePla
       if (stage == 1) {
         // X1^T[(tau,c),(a,Q)] = sum_d Grev^k[(tau,c),d] T[d,(a,Q)]                    (Algorithm 3 line 6)
         // column index n = (a, Q) with Q fastest: a tile row of C is then CONTIGUOUS in X1[tau][(c,a)][Q] (full-sector stores;
-        // X1 is written nt times per T element read, so the scattered side is the read of T[Q][d][a], 16-byte pieces n2 apart)
+        // and so is the operand row, read from the aux-last copy of T the library makes per push)
         S.a_off = (long long)k * ntau * gts;
-        S.am = lvl2(nao, gts, nao); S.ak = lvl1(1);
+        S.am = lvl2(nao, gts, 1); S.ak = lvl1(nao);          // A = the library's transposed copy Grev^T[tau][d][c]: c contiguous
         S.b_off = l * xs;
-        S.bk = lvl1(nao); S.bn = lvl2(naux, 1, n2);          // n = (a, Q): T[Q][d][a]
+        S.bk = lvl1((long long)nao * naux); S.bn = lvl1(1);  // n = (a, Q): the library's aux-last copy T'[d][a][Q] = T[Q][d][a]
         P.cm = lvl2(nao, xs, (long long)nao * naux);         // X1[tau][(c,a)][Q]
         P.cn = lvl1(1);                                      // a * naux + Q = n
         P.flags = 0;
@@ -922,9 +922,9 @@ int Plan::build_p0_stage(long long p0, long long np, int nt, int stage, StagePla
         // X2^T[(tau,a),(c,Q')] = sum_b G^{kq}[(tau,a),b] conj(T[Q'][c][b])              (Algorithm 3 line 7)
         // n = (c, Q') with Q' fastest, for the same reason: runs of naux contiguous elements of X2[tau][(c,a)][Q'] per tile row
         S.a_off = (long long)kq * ntau * gts;
-        S.am = lvl2(nao, gts, nao); S.ak = lvl1(1);
+        S.am = lvl2(nao, gts, 1); S.ak = lvl1(nao);          // A = the transposed copy G^T[tau][b][a]: a contiguous
         S.b_off = l * xs;
-        S.bk = lvl1(1); S.bn = lvl2(naux, nao, n2);          // n = (c, Q'): T[Q'][c][b]
+        S.bk = lvl1(naux); S.bn = lvl2(naux, (long long)nao * naux, 1);   // n = (c, Q'): the aux-last copy T'[c][b][Q'] = T[Q'][c][b]
         P.cm = lvl2(nao, xs, naux);                          // X2[tau][(c,a)][Q']: a * naux
         P.cn = lvl2(naux, (long long)nao * naux, 1);         // c * nao * naux + Q'
         P.flags = GWSIG_FLAG_CONJ_B;

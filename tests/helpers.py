@@ -275,14 +275,16 @@ def run_p0_plan_numpy(cfg, inp, G_flat, V_flat, push_pairs=None, nt=None):
         Gsrc = np.stack(Gs)
     else:
         Gsrc = G_flat.reshape(nk, ntau, nao, nao)
-    Grev = np.ascontiguousarray(Gsrc[:, ::-1]).ravel()          # G(beta - tau); the sign of G(-tau) = -G(beta - tau) is in the scale
-    Gsrc = np.ascontiguousarray(Gsrc).ravel()
+    # the library's two transposed copies: G(beta - tau)^T (the sign of G(-tau) = -G(beta - tau) is in the scale) and G(tau)^T
+    Grev = np.ascontiguousarray(Gsrc[:, ::-1].transpose(0, 1, 3, 2)).ravel()
+    Gsrc = np.ascontiguousarray(Gsrc.transpose(0, 1, 3, 2)).ravel()
     acc = np.zeros(nq * ntau * naux * naux, complex)
     xs = naux * nao * nao
     p0 = 0
     while p0 < npairs:
         npp = min(push_pairs, npairs - p0)
-        Vsub = V_flat[p0 * xs:(p0 + npp) * xs]
+        # the library's stage-1 / stage-2 descriptors address its aux-last copy T'[x][y][Q] = T[Q][x][y] of the pushed tensors
+        Vsub = np.ascontiguousarray(V_flat[p0 * xs:(p0 + npp) * xs].reshape(npp, naux, nao * nao).transpose(0, 2, 1)).ravel()
         for t0 in range(0, ntau, nt):
             ntc = min(nt, ntau - t0)
             X1 = np.zeros(npp * xs * ntc, complex)
