@@ -519,8 +519,9 @@ int Plan::build_stage(long long p0, long long np, int nt, int stage, int q_first
         p3.push_back(std::move(x));
       }
     }
-    // enough tiles for ~6 rounds of 2 CTAs per SM, pieces of at least ~512 k
-    const long long want = 12LL * std::max(num_sms, 1);
+    // enough tiles for ~12 rounds of 2 CTAs per SM, pieces of at least ~512 k (measured on cfg3, ms of stage 3 for 4 / 8 / 12 / 20 /
+    // 32 tiles per SM: 211 / 167 / 163 / 154.5 / 153.7)
+    const long long want = 24LL * std::max(num_sms, 1);
     for (auto& x : p3) {
       long long parts = tiles1 > 0 ? (want + tiles1 - 1) / tiles1 : 1;
       parts = std::max(1LL, std::min<long long>(parts, std::max(1LL, x.kt / 512)));
