@@ -532,9 +532,10 @@ def reference_main(args, rank, world):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
-# capture of this command (profiles/r2_ncu_default_engine_cfg3.md); ncu never runs inside bench.py, so every other
+# capture of this command (profiles/r2_ncu_default_engine_cfg3.md, r2_ncu_cfg4_stages12.md); ncu never runs inside bench.py, so every other
 # (workload, mode, engine) reports null.  Key: (workload, mode, engine option, stage index 0..2).
-NCU_DRAM_BYTES_PER_LAUNCH = {("cfg3", "ibz_block", 0, 1): 7.72e9}
+NCU_DRAM_BYTES_PER_LAUNCH = {("cfg3", "ibz_block", 0, 1): 7.72e9,
+                             ("cfg4", "ibz_block", 0, 1): 11.23e9}   # cfg4: a generic-q launch (profiles/r2_ncu_cfg4_stages12.md); launch sizes vary with q
 
 
 def main():
